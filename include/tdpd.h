@@ -1,0 +1,195 @@
+/*
+ * tdpd.h — C ABI of libtdpd.so: the per-timestep hot path of transport Dissipative Particle Dynamics
+ * (tDPD) with explicit red-blood-cell membranes (arXiv:1611.06163) on ONE NVIDIA B200 (sm_100a).
+ *
+ * Citations are /root/reference/PAPER.md:<line> (+ equation) and DESIGN.md readings R<n>.
+ *
+ * The path behind tdpd_step (every stage is a hand-written CUDA kernel; there is no CPU fallback):
+ *   a1-a3  cell-list binning: wrap + cell hash in Morton order, stable radix sort, cell-start table, reorder
+ *
+ *   a4     non-bonded pair kernel: F_i = sum_j [F^C + F^D + F^R] (Eq 2-6) for r < r_c and
+ *          Q_i = sum_j [Q^D + Q^R] (Eq 7-10) for r < r_cc, both sides of each pair, no atomics
+ *   a5-a8  membrane kernel: WLC+POW bonds with dissipative/random terms (Eq 13-16), K-Gather of
+ *          total area/volume and K-Apply of the area/volume constraints (Eq 17-18),
+ *          dihedral bending (Eq 19)
+ *   a9     fused velocity-Verlet of position, velocity and concentration (R21; the paper is silent)
+ *   a10    a4 and a5-a8 run on two caller-supplied CUDA streams joined by events
+ *
+ * Conventions
+ *   - All array arguments are HOST pointers, caller-owned, C-contiguous; the library copies in / out.
+ *     The only DEVICE pointer is the workspace given to tdpd_set_workspace (caller-owned device memory, e.g. a
+ *     torch uint8 tensor); the library owns its contents until tdpd_destroy.
+ *   - Particle ids are persistent: 0..n-1 in the order of the load/add calls.  Every get_* returns arrays in
+ *     id order regardless of the internal (cell-sorted) order.
+ *   - Every function returns TDPD_OK (0) or a negative error code; tdpd_last_error gives a message.
+ *     Nothing throws, aborts or prints across this boundary.
+ *   - One handle is used from one host thread at a time.
+ *   - Random numbers: Philox-4x32-10, counter = (min id, max id, step word k, tag), key = seed (DESIGN.md R-RNG).
+ *     Force evaluation number k uses step word k; the evaluation at load time is k = 0; after tdpd_step(n) the
+ *     step counter is n.  Results do not depend on how steps are batched.
+ */
+#ifndef TDPD_H
+#define TDPD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDPD_MAX_TYPES 4
+#define TDPD_MAX_SPECIES 4
+
+enum {
+  TDPD_OK = 0,
+  TDPD_EINVAL = -1,    /* bad argument, box smaller than 3 cells per axis, type out of range, open mesh ... */
+  TDPD_ESTATE = -2,    /* call order: step before workspace, load after workspace, ... */
+  TDPD_ENOMEM = -3,    /* workspace too small / allocation failed */
+  TDPD_ECUDA = -4,     /* a CUDA call failed; see tdpd_last_error */
+  TDPD_EUNSTABLE = -5  /* NaN / Inf in the state, or a WLC bond reached x >= 1, seen at tdpd_get_state */
+};
+
+enum { TDPD_BODY_OFF = 0, TDPD_BODY_UNIFORM = 1, TDPD_BODY_DOUBLE_POISEUILLE_Z = 2 };
+
+/* Model and run parameters (POD).  struct_size must be sizeof(tdpd_params). */
+typedef struct tdpd_params {
+  uint32_t struct_size;
+  int32_t n_types;    /* 1..TDPD_MAX_TYPES   */
+  int32_t n_species;  /* 1..TDPD_MAX_SPECIES */
+  float box[3];       /* periodic box lengths; >= 3 cells of edge max(r_c, r_cc) per axis */
+  float r_c;          /* force cutoff (Eq 3-5) */
+  float r_cc;         /* flux cutoff (Eq 8-9)  */
+  float dt;
+  float kBT;
+  float rho;          /* number density entering Eq 10 (R6) */
+  float a[TDPD_MAX_TYPES][TDPD_MAX_TYPES];      /* Eq 3 alpha_ij; must be symmetric */
+  float gamma[TDPD_MAX_TYPES][TDPD_MAX_TYPES];  /* Eq 4 gamma_ij; sigma_ij^2 = 2 kBT gamma_ij (Eq 6) */
+  float s_R[TDPD_MAX_TYPES][TDPD_MAX_TYPES];    /* omega_R = (1 - r/r_c)^s_R, omega_D = omega_R^2 (R3) */
+  float kappa[TDPD_MAX_SPECIES][TDPD_MAX_TYPES][TDPD_MAX_TYPES]; /* Eq 8 kappa_ij per species (R15) */
+  float s_c[TDPD_MAX_SPECIES];                  /* omega_DC = (1 - r/r_cc)^s_c (R4) */
+  float m_s[TDPD_MAX_SPECIES];                  /* Eq 10 m_s; 0 switches the random flux off */
+  float body_force[3];
+  int32_t body_mode;  /* TDPD_BODY_* (R14) */
+  uint64_t seed;
+  int32_t exclude_same_cell_membrane_pairs;     /* R16 */
+  int32_t reserved;
+} tdpd_params;
+
+/* Membrane model parameters (values are inputs, R11). */
+typedef struct tdpd_rbc_params {
+  float p;        /* WLC persistence length (Eq 13) */
+  float x0;       /* h_m / h_0 */
+  float m;        /* POW exponent (Eq 14) */
+  float gamma_T, gamma_C;   /* Eq 15; requires 3 gamma_C >= gamma_T (Eq 16) */
+  float k_g, k_l, k_v;      /* Eq 17-18 */
+  float k_b, theta0;        /* Eq 19 */
+  float VR_over_AR32;       /* V^R / (A^R)^{3/2} */
+} tdpd_rbc_params;
+
+typedef struct tdpd_sim tdpd_sim; /* opaque, library-owned */
+
+/* Creates an empty simulation on CUDA device `device`.  stream_pair / stream_bonded are caller-owned
+ * cudaStream_t handles (e.g. torch.cuda.Stream().cuda_stream); NULL selects library-created streams.
+ * EINVAL: bad struct_size / ranges / asymmetric tables / box too small. */
+int tdpd_create(const tdpd_params* p, int device, void* stream_pair, void* stream_bonded, tdpd_sim** out);
+
+/* Appends n free particles (position, velocity, concentration of every species).
+ * pos [n][3] inside [0, box) (values outside are wrapped once), vel [n][3] or NULL (zero), type [n] or NULL
+ * (type 0), conc [n][n_species] or NULL (zero).  ESTATE after tdpd_set_workspace. */
+int tdpd_load_particles(tdpd_sim* s, int64_t n, const float* pos, const float* vel, const int32_t* type,
+                        const float* conc);
+
+/* Appends one closed triangulated membrane: nv vertices (box coordinates, may straddle the
+ * periodic boundary), ntri triangles tri[ntri][3] of local vertex indices, counter-clockwise seen from outside.
+ * The library derives the bonds (unique edges), one dihedral per shared edge, per-bond rest length h_0 = initial
+ * length and k_p from force balance at h_0 (R11), per-triangle A_0t, A_0 = sum A_0t and
+ * V_0 = A_0^{3/2} V^R/(A^R)^{3/2}.  Vertices get particle type `mtype`.
+ * *rbc_index_out (may be NULL) receives the 0-based membrane index.
+ * EINVAL: mesh not a closed consistently oriented manifold, nv > 65535, 3 gamma_C < gamma_T. */
+int tdpd_add_rbc_mesh(tdpd_sim* s, int32_t nv, const float* verts, const float* vel, const float* conc,
+                      int32_t ntri, const int32_t* tri, const tdpd_rbc_params* rp, int32_t mtype,
+                      int32_t* rbc_index_out);
+
+/* Device bytes needed for everything loaded so far. */
+int tdpd_workspace_bytes(const tdpd_sim* s, size_t* bytes);
+
+/* Hands the library its device memory (256-byte aligned, >= tdpd_workspace_bytes) and uploads the system.
+ * dev_ptr == NULL: the library allocates with cudaMalloc and frees at destroy.  After this call the particle
+ * set is frozen.  ENOMEM: too small. */
+int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes);
+
+/* Replaces the parameters; takes effect at the next force evaluation (the current forces are re-evaluated with
+ * the current step word before the next step).  The cell grid and the type/species counts must not change
+ * after tdpd_set_workspace (EINVAL). */
+int tdpd_set_params(tdpd_sim* s, const tdpd_params* p);
+
+/* Overwrites positions / velocities / concentrations of all particles in id order (any pointer may be NULL),
+ * keeps the step counter.  Forces are re-evaluated with the current step word. */
+int tdpd_set_state(tdpd_sim* s, const float* pos, const float* vel, const float* conc);
+
+/* Advances nsteps velocity-Verlet steps (R21).  Asynchronous: only enqueues work on the two streams. */
+int tdpd_step(tdpd_sim* s, int32_t nsteps);
+
+/* Blocks until all enqueued work is done. */
+int tdpd_sync(tdpd_sim* s);
+
+/* Copies out, in id order: pos [n][3], vel [n][3], conc [n][S], force [n][3] (pair + bonded, without the body
+ * term), flux [n][S], *step.  Any pointer may be NULL.  Synchronises.  EUNSTABLE if a value is not finite. */
+int tdpd_get_state(tdpd_sim* s, float* pos, float* vel, float* conc, float* force, float* flux, int64_t* step);
+
+/* Same as the force part of tdpd_get_state, split into the non-bonded and the membrane contribution. */
+int tdpd_get_forces_split(tdpd_sim* s, float* force_pair, float* force_bonded);
+
+int64_t tdpd_num_particles(const tdpd_sim* s);
+int32_t tdpd_num_rbc(const tdpd_sim* s);
+
+/* Per membrane: total area and volume of the last force evaluation (K-Gather) and the targets.
+ * Any pointer may be NULL.  Synchronises. */
+int tdpd_get_rbc_stats(tdpd_sim* s, double* area, double* volume, double* A0, double* V0);
+
+/* Derived topology of membrane m (for tests): nbond, then bond[nbond][2], dih[nbond][4], h0, kp (per bond),
+ * A0t (per triangle); any array may be NULL. */
+int tdpd_get_rbc_topology(tdpd_sim* s, int32_t m, int32_t* nbond, int32_t* bond, int32_t* dih, float* h0,
+                          float* kp, float* A0t);
+
+/* Binning of the current positions (bit-exact test, DESIGN.md R-bin): cell_xyz [n][3] by id,
+ * ncell[3], cell_count [ncell_x*ncell_y*ncell_z] x-fastest (may be NULL), and sorted_id [n]: the id held by each
+ * slot of the cell-sorted order (may be NULL). */
+int tdpd_debug_get_binning(tdpd_sim* s, int32_t* cell_xyz, int32_t ncell[3], int32_t* cell_count,
+                           int32_t* sorted_id);
+
+/* Neighbour census through the cell list of the current positions (exact arithmetic on the fp32 positions):
+ * per id the number of neighbours within r_c and r_cc and the XOR of their ids (same-membrane pairs and
+ * coincident particles excluded exactly as in the force sum). */
+int tdpd_debug_neighbor_census(tdpd_sim* s, int32_t* n_rc, int32_t* n_rcc, uint32_t* xor_rc, uint32_t* xor_rcc);
+
+/* Raw random stream of the device path (for the bit-exact Philox test and the Gaussian tolerance test):
+ * words [n][4] = Philox-4x32-10 of counter (min(id_i,id_j), max(id_i,id_j), step, tag) with the simulation's
+ * seed; gauss [n][4] = the four Gaussians the kernels derive from them (fp32).  Either may be NULL. */
+int tdpd_debug_rng(tdpd_sim* s, int64_t n, const int64_t* id_i, const int64_t* id_j, int64_t step, uint32_t tag,
+                   uint32_t* words, float* gauss);
+
+/* Per-kernel timing with CUDA events on the launching streams (bench.py's roofline leg).  While enabled every
+ * launch of the kernels below is bracketed by an event pair; tdpd_get_timing synchronises and returns, per
+ * kernel class, the number of launches and the summed milliseconds since tdpd_set_timing(s, 1).
+ * Classes: 0 integrate (kick/drift/key), 1 sort, 2 reorder + cell table, 3 pair, 4 membrane, 5 closing kick. */
+#define TDPD_N_TIMERS 6
+int tdpd_set_timing(tdpd_sim* s, int32_t on);
+int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], double ms[TDPD_N_TIMERS]);
+
+/* Number of kernels the library launched since creation (bench.py's gpu_launches). */
+int64_t tdpd_launch_count(const tdpd_sim* s);
+
+/* Pair-kernel configuration knobs (tuning; results are identical up to fp32 summation order within a cell):
+ * brick_log2 in 3..5 = cells per CTA brick (2x2x2, 4x2x2, 4x4x2); 0 = automatic.  use_graph: capture the
+ * step into a CUDA graph. */
+int tdpd_set_tuning(tdpd_sim* s, int32_t brick_log2, int32_t use_graph);
+
+const char* tdpd_last_error(const tdpd_sim* s);
+int tdpd_destroy(tdpd_sim* s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDPD_H */

@@ -1,0 +1,189 @@
+// binning.cu — rows a2 and a3 of SURVEY §8(a): stable LSD radix sort of (cell key, previous slot) and the
+// reorder + cell-start table (PAPER.md:137 "particle reordering", :141 "radix sort").  No atomics decide an
+// order anywhere, so the sorted order (and with it every fp32 summation order downstream) is deterministic.
+#include "common.cuh"
+
+namespace {
+constexpr int RB = 8;            // bits per pass
+constexpr int NBIN = 1 << RB;
+constexpr int SORT_NT = 256;     // 8 warps
+constexpr int SORT_ITEMS = 16;   // keys per thread
+constexpr int TILE = SORT_NT * SORT_ITEMS;
+constexpr int WCHUNK = 32 * SORT_ITEMS;  // contiguous keys owned by one warp
+
+// per-tile digit histogram -> hist[bin * nblk + blk]  (integer counts: atomics cannot change the result)
+__global__ void __launch_bounds__(SORT_NT) k_sort_hist(const uint32_t* __restrict__ keys, int64_t n, int shift,
+                                                       uint32_t* __restrict__ hist, int nblk) {
+  __shared__ uint32_t cnt[NBIN];
+  cnt[threadIdx.x] = 0;
+  __syncthreads();
+  int64_t base = (int64_t)blockIdx.x * TILE;
+#pragma unroll 4
+  for (int it = 0; it < SORT_ITEMS; ++it) {
+    int64_t i = base + it * SORT_NT + threadIdx.x;
+    if (i < n) atomicAdd(&cnt[(keys[i] >> shift) & (NBIN - 1)], 1u);
+  }
+  __syncthreads();
+  hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
+}
+
+// exclusive scan of hist[0..total) by one CTA of 1024 threads
+__global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ hist, int64_t total) {
+  __shared__ uint32_t wsum[32];
+  __shared__ uint32_t carry_s;
+  int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int64_t base = 0; base < total; base += 4096) {
+    int64_t i0 = base + (int64_t)threadIdx.x * 4;
+    uint32_t v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = (i0 + k < total) ? hist[i0 + k] : 0u;
+    uint32_t tsum = v[0] + v[1] + v[2] + v[3];
+    uint32_t x = tsum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      uint32_t y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    if (w == 0) {
+      uint32_t s = wsum[lane];
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        uint32_t y = __shfl_up_sync(0xffffffffu, s, d);
+        if (lane >= d) s += y;
+      }
+      wsum[lane] = s;  // inclusive over warps
+    }
+    __syncthreads();
+    uint32_t carry = carry_s;
+    uint32_t excl = carry + (w ? wsum[w - 1] : 0u) + (x - tsum);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (i0 + k < total) hist[i0 + k] = excl;
+      excl += v[k];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) carry_s = carry + wsum[31];
+    __syncthreads();
+  }
+}
+
+// stable scatter: tile order = (warp, item, lane); rank = scanned tile base + keys of the same digit in earlier
+// warps of the tile + earlier keys of the same digit in this warp
+__global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __restrict__ kin,
+                                                          const uint32_t* __restrict__ vin,
+                                                          uint32_t* __restrict__ kout, uint32_t* __restrict__ vout,
+                                                          int64_t n, int shift, const uint32_t* __restrict__ hist,
+                                                          int nblk) {
+  __shared__ uint32_t wbase[SORT_NT / 32][NBIN];
+  int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int k = threadIdx.x; k < (SORT_NT / 32) * NBIN; k += SORT_NT) (&wbase[0][0])[k] = 0;
+  __syncthreads();
+  int64_t base = (int64_t)blockIdx.x * TILE + (int64_t)w * WCHUNK;
+  uint32_t key[SORT_ITEMS];
+#pragma unroll
+  for (int it = 0; it < SORT_ITEMS; ++it) {
+    int64_t i = base + it * 32 + lane;
+    key[it] = i < n ? kin[i] : 0xFFFFFFFFu;
+    if (i < n) atomicAdd(&wbase[w][(key[it] >> shift) & (NBIN - 1)], 1u);
+  }
+  __syncthreads();
+  {  // per bin: counts -> exclusive prefix over warps + global base
+    int b = threadIdx.x;
+    uint32_t run = hist[(int64_t)b * nblk + blockIdx.x];
+#pragma unroll
+    for (int ww = 0; ww < SORT_NT / 32; ++ww) {
+      uint32_t c = wbase[ww][b];
+      wbase[ww][b] = run;
+      run += c;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int it = 0; it < SORT_ITEMS; ++it) {
+    int64_t i = base + it * 32 + lane;
+    bool valid = i < n;
+    uint32_t d = valid ? ((key[it] >> shift) & (NBIN - 1)) : 0xFFFFu;
+    uint32_t peers = __match_any_sync(0xffffffffu, d);
+    uint32_t rank = __popc(peers & ((1u << lane) - 1u));
+    uint32_t dest = 0;
+    if (valid) dest = wbase[w][d] + rank;
+    __syncwarp();
+    if (valid && rank == 0) wbase[w][d] += __popc(peers);
+    __syncwarp();
+    if (valid) {
+      kout[dest] = key[it];
+      vout[dest] = vin[i];
+    }
+  }
+}
+
+// gather the state into the new order, record slot_of_id for membrane vertices, fill the cell-start table
+template <int S>
+__global__ void __launch_bounds__(256) k_reorder(SortedState src, SortedState dst, const uint32_t* __restrict__ keys,
+                                                 const uint32_t* __restrict__ vals, int64_t n, uint32_t ncell,
+                                                 uint32_t* __restrict__ cell_start, uint32_t* __restrict__ slot_of_id) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  uint32_t k = keys[i];
+  uint32_t from = vals[i];
+  float4 p = src.pos[from];
+  float4 v = src.vel[from];
+  uint32_t m = src.meta[from];
+  dst.pos[i] = p;
+  dst.vel[i] = v;
+  dst.meta[i] = m;
+#pragma unroll
+  for (int s = 1; s < S; ++s) dst.cx[(int64_t)(s - 1) * n + i] = src.cx[(int64_t)(s - 1) * n + from];
+  if (m >> 2) slot_of_id[__float_as_uint(p.w)] = (uint32_t)i;
+  // cell_start[r] = first slot whose key >= r
+  uint32_t kprev = i == 0 ? 0u : keys[i - 1] + 1u;
+  if (i == 0 || keys[i - 1] != k)
+    for (uint32_t r = kprev; r <= k; ++r) cell_start[r] = (uint32_t)i;
+  if (i == n - 1)
+    for (uint32_t r = k + 1; r <= ncell; ++r) cell_start[r] = (uint32_t)n;
+}
+}  // namespace
+
+int td_sort_passes(int key_bits) { return key_bits <= 0 ? 1 : (key_bits + RB - 1) / RB; }
+
+size_t td_sort_scratch_bytes(int64_t n) {
+  int64_t nblk = (n + TILE - 1) / TILE;
+  if (nblk < 1) nblk = 1;
+  return (size_t)nblk * NBIN * sizeof(uint32_t);
+}
+
+int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits, void* scratch, cudaStream_t st,
+                   int* n_launches) {
+  int side = 0;
+  if (n == 0) return side;
+  int nblk = (int)((n + TILE - 1) / TILE);
+  uint32_t* hist = (uint32_t*)scratch;
+  int passes = td_sort_passes(key_bits);
+  for (int p = 0; p < passes; ++p) {
+    int shift = p * RB;
+    k_sort_hist<<<nblk, SORT_NT, 0, st>>>(keys[side], n, shift, hist, nblk);
+    k_sort_scan<<<1, 1024, 0, st>>>(hist, (int64_t)nblk * NBIN);
+    k_sort_scatter<<<nblk, SORT_NT, 0, st>>>(keys[side], vals[side], keys[side ^ 1], vals[side ^ 1], n, shift, hist,
+                                              nblk);
+    side ^= 1;
+    if (n_launches) *n_launches += 3;
+  }
+  return side;
+}
+
+void td_launch_reorder(const SortedState& src, const SortedState& dst, const uint32_t* keys, const uint32_t* vals,
+                       int64_t n, int n_species, uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id,
+                       cudaStream_t st) {
+  if (n == 0) return;
+  int nb = (int)((n + 255) / 256);
+  switch (n_species) {
+    case 1: k_reorder<1><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
+    case 2: k_reorder<2><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
+    case 3: k_reorder<3><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
+    default: k_reorder<4><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
+  }
+}

@@ -1,0 +1,176 @@
+// common.cuh — device-side structures shared by the kernels of libtdpd.so (CUDA path only; nothing here is
+// shared with oracle/).  Citations: /root/reference/PAPER.md:<line>, readings R<n>.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define TD_T 4  // max particle types
+#define TD_S 4  // max species
+
+// Parameters in the form the kernels consume (derived once on the host from tdpd_params).
+struct DevParams {
+  int n_types, n_species;
+  float box[3];
+  float half_box_z;
+  int ncell[3];
+  float cell_inv[3];   // (float)(n_a / L_a): binning multiplier (R-bin)
+  float cell_edge[3];  // L_a / n_a
+  float r_c, r_cc, rc2, rcc2, rcut2, inv_rc, inv_rcc;
+  float dt, half_dt;
+  // type-pair tables, index ti*TD_T + tj
+  float a[TD_T * TD_T];
+  float gamma[TD_T * TD_T];
+  float sig[TD_T * TD_T];  // sqrt(2 kBT gamma) / sqrt(dt)   (Eq 5-6)
+  float s_R[TD_T * TD_T];
+  float kappa[TD_S][TD_T * TD_T];
+  float epsc[TD_S];  // m_s^2 rho / dt: Q^R = sgn zeta w_RC sqrt(kappa (Ci+Cj) epsc)  (Eq 9-10)
+  float s_c[TD_S];
+  float body[3];
+  int body_mode;
+  uint32_t key0[10], key1[10];  // Philox round keys: seed + r * Weyl
+  int excl_same;
+  int fast_w;     // every s_R == 0.5 and every s_c == 2: weights need no pow
+  int rand_flux;  // some m_s != 0
+};
+
+// meta word of a particle: bits 0-1 type, bits 2-31 membrane id + 1 (0 = free particle)
+__host__ __device__ inline uint32_t td_meta(int type, int rbc1) { return (uint32_t)type | ((uint32_t)rbc1 << 2); }
+
+// ---- Philox-4x32-10 (Salmon et al. SC'11; DESIGN.md R-RNG) -----------------------------------------------
+// counter (c0,c1,c2,c3), round keys precomputed in DevParams.
+__device__ __forceinline__ void td_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t* k0,
+                                          const uint32_t* k1, uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0[r];
+    uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1[r];
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+    c0 = n0;
+    c2 = n2;
+  }
+  o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+
+// word -> uniform strictly inside (0,1): u = ((x >> 9) + 1/2) 2^-23 (exact in fp32)
+__device__ __forceinline__ float td_uniform(uint32_t x) {
+  return fmaf((float)(x >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
+}
+
+// Box-Muller: R = sqrt(-2 ln ua); (g_cos, g_sin) = R (cos 2 pi ub, sin 2 pi ub).
+// MUFU lg2/sin/cos; lg2.approx has absolute error 2^-22 on (0.5, 2), which is not good enough for R when
+// ua -> 1 (R -> 0), so the top 2^-17 of the range uses the series -2 ln(1 - t) = 2t + t^2 + O(t^3).
+__device__ __forceinline__ void td_box_muller(uint32_t xa, uint32_t xb, float& g_cos, float& g_sin) {
+  float q;
+  if (xa >= 0xFFFF8000u) {
+    // t = 1 - ua = ((2^23 - 1 - (xa >> 9)) + 1/2) 2^-23, exact
+    float t = fmaf((float)(8388607u - (xa >> 9)), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
+    q = fmaf(t, t, 2.0f * t);
+  } else {
+    q = -1.3862943611198906f * __log2f(td_uniform(xa));  // -2 ln 2 * lg2(u)
+  }
+  float R = sqrtf(q);
+  float ang = 6.283185307179586f * td_uniform(xb);
+  g_cos = R * __cosf(ang);
+  g_sin = R * __sinf(ang);
+}
+
+// ---- kernel argument blocks -----------------------------------------------------------------------------
+struct SortedState {   // one side of the ping-pong, cell-sorted order
+  float4* pos;     // x, y, z, id (bits)
+  float4* vel;     // vx, vy, vz, C_0
+  float* cx;       // [(S-1)][n]: C_1.. species-major
+  uint32_t* meta;  // td_meta
+};
+
+struct Brick {  // one CTA of the pair kernel: 2^k consecutive Morton codes
+  int ox, oy, oz;       // cell coordinates of the brick origin
+  uint32_t r0, ncell;   // first Morton rank, number of existing cells
+};
+
+struct PairArgs {
+  SortedState st;
+  const uint32_t* cell_start;  // [ncell + 1] by Morton rank
+  const uint32_t* cell_rank;   // [ncell] x-fastest linear cell -> Morton rank
+  const uint32_t* rank_cell;   // [ncell] Morton rank -> packed cx | cy << 10 | cz << 20
+  const Brick* bricks;
+  float4* F4;                  // Fx, Fy, Fz, Q_0 by slot
+  float* Qx;                   // [(S-1)][n]
+  int64_t n;
+  uint32_t step;               // RNG step word
+  int bx, by, bz;              // brick dims in cells
+  int hcap, lcap;              // smem capacities: halo particles, list entries per thread
+  int* err;                    // device error word
+};
+
+// mesh template (topology shared by all membranes with the same triangle list), CSR per vertex
+struct MeshTemplateDev {
+  int nv, ntri, nbond;
+  const uint16_t* tri;    // [ntri][3]
+  const uint16_t* dih;    // [nbond][4]
+  const int* voff;        // [nv + 1]
+  const uint32_t* vbond;  // [2 nbond]: neighbour vertex | bond index << 16
+  const uint32_t* vtri;   // [3 ntri]: triangle | role << 16
+  const int* vdoff;       // [nv + 1]
+  const uint32_t* vdih;   // [4 nbond]: dihedral | role << 16
+};
+
+struct RbcDev {
+  int64_t first_id;
+  int tmpl;
+  int data_off;  // offset of this membrane's h0/kp (per bond) arrays
+  int tri_off;   // offset of A0t
+  float A0, V0;
+  float kBT_over_p, inv_x0, m_pow, gamma_T, gamma_C, k_g, k_l, k_v, k_b, cos_t0, sin_t0;
+  float rnd_T, rnd_C;  // sqrt(2 kBT/dt) sqrt(2 gT), sqrt(2 kBT/dt) sqrt(3 gC - gT)/3
+};
+
+struct MembraneArgs {
+  SortedState st;
+  const uint32_t* slot_of_id;
+  const RbcDev* rbcs;
+  const MeshTemplateDev* tmpls;
+  const float* h0;
+  const float* kp;
+  const float* A0t;
+  float4* Fb;       // bonded force by id
+  double* stats;    // [M][2] area, volume
+  int nchunk;       // CTAs per membrane
+  uint32_t step;
+  int* err;
+};
+
+enum { TD_ERR_HALO_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4 };
+
+// ---- launchers (each .cu exposes host functions; all launches are asynchronous on `st`) -------------------
+void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
+                         const uint32_t* cell_rank, cudaStream_t st);
+void td_launch_kick_drift_key(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
+                              const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
+                              bool closing_first, cudaStream_t st);
+void td_launch_kick(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx, const float4* Fb,
+                    int64_t n, cudaStream_t st);
+int td_sort_passes(int key_bits);
+size_t td_sort_scratch_bytes(int64_t n);
+// sorts (keys, vals); result ends in keys[out_side]/vals[out_side]; returns out_side
+int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits, void* scratch, cudaStream_t st,
+                   int* n_launches);
+void td_launch_reorder(const SortedState& src, const SortedState& dst, const uint32_t* keys, const uint32_t* vals,
+                       int64_t n, int n_species, uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id,
+                       cudaStream_t st);
+int td_launch_pair(const DevParams& P, const PairArgs& A, int nbricks, int nthreads, cudaStream_t st);
+size_t td_pair_smem_bytes(int n_species, int bx, int by, int bz, int hcap, int lcap, int nthreads);
+int td_launch_membrane(const DevParams& P, const MembraneArgs& A, int n_rbc, int max_nv, int nthreads,
+                       cudaStream_t st);
+void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, const float4* Fb, int64_t n,
+                      int n_species, int what, float* out, int* err, cudaStream_t st);
+void td_launch_set_state(const DevParams& P, const SortedState& s, int64_t n, const float* pos, const float* vel,
+                         const float* conc, cudaStream_t st);
+void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, int32_t* cell_xyz,
+                             int32_t* cell_count, int32_t* sorted_id, cudaStream_t st);
+void td_launch_census(const DevParams& P, const SortedState& s, const uint32_t* cell_start, const uint32_t* cell_rank,
+                      int64_t n, int32_t* n_rc, int32_t* n_rcc, uint32_t* xor_rc, uint32_t* xor_rcc, cudaStream_t st);
+void td_launch_rng_debug(const DevParams& P, int64_t n, const int64_t* id_i, const int64_t* id_j, uint32_t step,
+                         uint32_t tag, uint32_t* words, float* gauss, cudaStream_t st);

@@ -1,0 +1,115 @@
+// integrate.cu — rows a1 and a9 of SURVEY §8(a): velocity-Verlet half-kicks of velocity and concentration, drift,
+// periodic wrap and the cell hash, fused (R21; BASELINE north_star (4) — the paper does not describe
+// its integrator).  Runs in the cell-sorted order of the previous binning.
+#include "common.cuh"
+
+// cell coordinate along one axis (DESIGN.md R-bin): c = min(n-1, floor(x * inv)), one rounded fp32 multiply
+__device__ __forceinline__ int td_cell_axis(float x, float inv, int n) {
+  int c = (int)floorf(__fmul_rn(x, inv));
+  c = c > n - 1 ? n - 1 : c;
+  return c < 0 ? 0 : c;
+}
+
+__device__ __forceinline__ float td_wrap(float x, float L) {
+  if (x >= L) x -= L;
+  if (x < 0.0f) {
+    x += L;
+    if (x >= L) x = 0.0f;  // x was a tiny negative number: its image is L == 0
+  }
+  return x;
+}
+
+__device__ __forceinline__ uint32_t td_key_of(const DevParams& P, float x, float y, float z,
+                                              const uint32_t* __restrict__ cell_rank) {
+  int cx = td_cell_axis(x, P.cell_inv[0], P.ncell[0]);
+  int cy = td_cell_axis(y, P.cell_inv[1], P.ncell[1]);
+  int cz = td_cell_axis(z, P.cell_inv[2], P.ncell[2]);
+  return __ldg(&cell_rank[(cz * P.ncell[1] + cy) * P.ncell[0] + cx]);
+}
+
+// body acceleration sign at the force-evaluation position (R14)
+__device__ __forceinline__ float td_body_sign(const DevParams& P, float z) {
+  if (P.body_mode == 1) return 1.0f;
+  if (P.body_mode == 2) return z < P.half_box_z ? 1.0f : -1.0f;
+  return 0.0f;
+}
+
+template <int S>
+__device__ __forceinline__ void td_half_kick(const DevParams& P, float4& p, float4& v, float* cx_val,
+                                             const float4* __restrict__ F4, const float* __restrict__ Qx,
+                                             const float4* __restrict__ Fb, uint32_t meta, int64_t i, int64_t n) {
+  float4 f = F4[i];
+  if (meta >> 2) {  // membrane vertex: add the bonded force (stored by id)
+    float4 b = Fb[__float_as_uint(p.w)];
+    f.x += b.x; f.y += b.y; f.z += b.z;
+  }
+  float sg = td_body_sign(P, p.z);
+  float h = P.half_dt;
+  v.x = fmaf(h, f.x + sg * P.body[0], v.x);
+  v.y = fmaf(h, f.y + sg * P.body[1], v.y);
+  v.z = fmaf(h, f.z + sg * P.body[2], v.z);
+  v.w = fmaf(h, f.w, v.w);
+#pragma unroll
+  for (int s = 1; s < S; ++s) cx_val[s - 1] = fmaf(h, Qx[(int64_t)(s - 1) * n + i], cx_val[s - 1]);
+}
+
+// mode: 0 = keys only (initial binning), 1 = opening half-kick + drift + wrap + key,
+//       2 = closing half-kick of the previous step, then mode 1, 3 = closing half-kick only
+template <int S>
+__global__ void __launch_bounds__(256) k_integrate(const DevParams P, SortedState st, const float4* __restrict__ F4,
+                                                   const float* __restrict__ Qx, const float4* __restrict__ Fb,
+                                                   int64_t n, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
+                                                   const uint32_t* __restrict__ cell_rank, int mode) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float4 p = st.pos[i];
+  if (mode != 0) {
+    float4 v = st.vel[i];
+    uint32_t meta = st.meta[i];
+    float cxv[S > 1 ? S - 1 : 1];
+#pragma unroll
+    for (int s = 1; s < S; ++s) cxv[s - 1] = st.cx[(int64_t)(s - 1) * n + i];
+    if (mode >= 2) td_half_kick<S>(P, p, v, cxv, F4, Qx, Fb, meta, i, n);
+    if (mode <= 2) {
+      td_half_kick<S>(P, p, v, cxv, F4, Qx, Fb, meta, i, n);
+      p.x = td_wrap(fmaf(P.dt, v.x, p.x), P.box[0]);
+      p.y = td_wrap(fmaf(P.dt, v.y, p.y), P.box[1]);
+      p.z = td_wrap(fmaf(P.dt, v.z, p.z), P.box[2]);
+      st.pos[i] = p;
+    }
+    st.vel[i] = v;
+#pragma unroll
+    for (int s = 1; s < S; ++s) st.cx[(int64_t)(s - 1) * n + i] = cxv[s - 1];
+  }
+  if (mode <= 2) {
+    keys[i] = td_key_of(P, p.x, p.y, p.z, cell_rank);
+    vals[i] = (uint32_t)i;
+  }
+}
+
+static void launch_integrate(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
+                             const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
+                             int mode, cudaStream_t st) {
+  if (n == 0) return;
+  int nb = (int)((n + 255) / 256);
+  switch (P.n_species) {
+    case 1: k_integrate<1><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
+    case 2: k_integrate<2><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
+    case 3: k_integrate<3><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
+    default: k_integrate<4><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
+  }
+}
+
+void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
+                         const uint32_t* cell_rank, cudaStream_t st) {
+  launch_integrate(P, s, nullptr, nullptr, nullptr, n, keys, vals, cell_rank, 0, st);
+}
+void td_launch_kick_drift_key(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
+                              const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
+                              bool closing_first, cudaStream_t st) {
+  launch_integrate(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, closing_first ? 2 : 1, st);
+}
+void td_launch_kick(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx, const float4* Fb,
+                    int64_t n, cudaStream_t st) {
+  launch_integrate(P, s, F4, Qx, Fb, n, nullptr, nullptr, nullptr, 3, st);
+}
