@@ -317,6 +317,10 @@ extern "C" int tdpd_add_rbc_mesh(tdpd_sim* s, int32_t nv, const float* verts, co
       double d = x - x0;
       r[3 * v + a] = x0 + (d - L * std::floor(d / L + 0.5));
     }
+  for (int v = 0; v < nv; ++v)
+    for (int a = 0; a < 3; ++a)
+      if (std::fabs(r[3 * v + a] - r[a]) >= 0.49 * (double)s->prm.box[a])
+        return fail(s, TDPD_EINVAL, "membrane extent must stay below half the box (minimum-image unwrap)");
   double kBT = s->prm.kBT, x0r = 1.0 / (double)rp->x0;
   double om = 1.0 - x0r;
   double f0 = kBT / (double)rp->p * (0.25 / (om * om) - 0.25 + x0r);  // dU_WLC/dh at h = h_0 (Eq 13)
@@ -431,7 +435,7 @@ static size_t layout(tdpd_sim* s, void* basep) {
     s->st[k].pos = c.take<float4>(n);
     s->st[k].vel = c.take<float4>(n);
     s->st[k].cx = c.take<float>(n * (size_t)std::max(S - 1, 1));
-    s->st[k].meta = c.take<uint32_t>(n);
+    s->st[k].lo = c.take<float4>(n);
     s->keys[k] = c.take<uint32_t>(n);
     s->vals[k] = c.take<uint32_t>(n);
   }
@@ -493,8 +497,7 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
   CK(cudaMemsetAsync(s->ws, 0, need, q));
   // particle state in id order = initial "sorted" side 0
   {
-    std::vector<float4> hp(n), hv(n);
-    std::vector<uint32_t> hm(n);
+    std::vector<float4> hp(n), hv(n), hm(n);
     std::vector<float> hc((size_t)std::max(S - 1, 1) * std::max<int64_t>(n, 1));
     for (int64_t i = 0; i < n; ++i) {
       uint32_t idb = (uint32_t)i;
@@ -502,13 +505,16 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
       memcpy(&idf, &idb, 4);
       hp[i] = make_float4(s->h_pos[3 * i], s->h_pos[3 * i + 1], s->h_pos[3 * i + 2], idf);
       hv[i] = make_float4(s->h_vel[3 * i], s->h_vel[3 * i + 1], s->h_vel[3 * i + 2], s->h_conc[(size_t)S * i]);
-      hm[i] = td_meta(s->h_type[i], s->h_rbc[i]);
+      uint32_t mb = td_meta(s->h_type[i], s->h_rbc[i]);
+      float mf;
+      memcpy(&mf, &mb, 4);
+      hm[i] = make_float4(0.f, 0.f, 0.f, mf);
       for (int sp = 1; sp < S; ++sp) hc[(size_t)(sp - 1) * n + i] = s->h_conc[(size_t)S * i + sp];
     }
     if (n) {
       CK(cudaMemcpyAsync(s->st[0].pos, hp.data(), n * sizeof(float4), cudaMemcpyHostToDevice, q));
       CK(cudaMemcpyAsync(s->st[0].vel, hv.data(), n * sizeof(float4), cudaMemcpyHostToDevice, q));
-      CK(cudaMemcpyAsync(s->st[0].meta, hm.data(), n * sizeof(uint32_t), cudaMemcpyHostToDevice, q));
+      CK(cudaMemcpyAsync(s->st[0].lo, hm.data(), n * sizeof(float4), cudaMemcpyHostToDevice, q));
       if (S > 1) CK(cudaMemcpyAsync(s->st[0].cx, hc.data(), (size_t)(S - 1) * n * sizeof(float), cudaMemcpyHostToDevice, q));
     }
     CK(cudaStreamSynchronize(q));

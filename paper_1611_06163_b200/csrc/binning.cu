@@ -132,10 +132,11 @@ __global__ void __launch_bounds__(256) k_reorder(SortedState src, SortedState ds
   uint32_t from = vals[i];
   float4 p = src.pos[from];
   float4 v = src.vel[from];
-  uint32_t m = src.meta[from];
+  float4 l = src.lo[from];
+  uint32_t m = __float_as_uint(l.w);
   dst.pos[i] = p;
   dst.vel[i] = v;
-  dst.meta[i] = m;
+  dst.lo[i] = l;
 #pragma unroll
   for (int s = 1; s < S; ++s) dst.cx[(int64_t)(s - 1) * n + i] = src.cx[(int64_t)(s - 1) * n + from];
   if (m >> 2) slot_of_id[__float_as_uint(p.w)] = (uint32_t)i;

@@ -82,7 +82,7 @@ struct SortedState {   // one side of the ping-pong, cell-sorted order
   float4* pos;     // x, y, z, id (bits)
   float4* vel;     // vx, vy, vz, C_0
   float* cx;       // [(S-1)][n]: C_1.. species-major
-  uint32_t* meta;  // td_meta
+  float4* lo;      // low-order words of x, y, z (position = pos + lo, two-float), td_meta (bits)
 };
 
 struct Brick {  // one CTA of the pair kernel: 2^k consecutive Morton codes

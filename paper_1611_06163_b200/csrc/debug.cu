@@ -16,7 +16,7 @@ __global__ void __launch_bounds__(256) k_unsort(SortedState st, const float4* __
   int64_t id = __float_as_uint(p.w);
   float v[4] = {0.f, 0.f, 0.f, 0.f};
   int cnt = 3;
-  if (what == 0) { v[0] = p.x; v[1] = p.y; v[2] = p.z; }
+  if (what == 0) { float4 l = st.lo[i]; v[0] = p.x + l.x; v[1] = p.y + l.y; v[2] = p.z + l.z; }
   else if (what == 1) { float4 w = st.vel[i]; v[0] = w.x; v[1] = w.y; v[2] = w.z; }
   else if (what == 2) {
     cnt = S;
@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(256) k_unsort(SortedState st, const float4* __
     for (int s = 1; s < S; ++s) v[s] = st.cx[(int64_t)(s - 1) * n + i];
   } else if (what == 3 || what == 5 || what == 6) {
     if (what != 6) { float4 f = F4[i]; v[0] = f.x; v[1] = f.y; v[2] = f.z; }
-    if (what != 5 && (st.meta[i] >> 2)) { float4 b = Fb[id]; v[0] += b.x; v[1] += b.y; v[2] += b.z; }
+    if (what != 5 && (__float_as_uint(st.lo[i].w) >> 2)) { float4 b = Fb[id]; v[0] += b.x; v[1] += b.y; v[2] += b.z; }
   } else {
     cnt = S;
     v[0] = F4[i].w;
@@ -70,7 +70,8 @@ __global__ void __launch_bounds__(128) k_census(const DevParams P, SortedState s
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float4 p = st.pos[i];
-  uint32_t mi = st.meta[i];
+  float4 pl = st.lo[i];
+  uint32_t mi = __float_as_uint(pl.w);
   int64_t id = __float_as_uint(p.w);
   int c[3] = {cell_axis(p.x, P.cell_inv[0], P.ncell[0]), cell_axis(p.y, P.cell_inv[1], P.ncell[1]),
               cell_axis(p.z, P.cell_inv[2], P.ncell[2])};
@@ -86,9 +87,11 @@ __global__ void __launch_bounds__(128) k_census(const DevParams P, SortedState s
         for (uint32_t k = cell_start[r]; k < cell_start[r + 1]; ++k) {
           if (k == i) continue;
           float4 q = st.pos[k];
-          uint32_t mj = st.meta[k];
+          float4 ql = st.lo[k];
+          uint32_t mj = __float_as_uint(ql.w);
           if (P.excl_same && (mi >> 2) && (mi >> 2) == (mj >> 2)) continue;
-          double d[3] = {(double)p.x - (double)q.x, (double)p.y - (double)q.y, (double)p.z - (double)q.z};
+          double d[3] = {((double)p.x + pl.x) - ((double)q.x + ql.x), ((double)p.y + pl.y) - ((double)q.y + ql.y),
+                         ((double)p.z + pl.z) - ((double)q.z + ql.z)};
           double r2 = 0.0;
           for (int k2 = 0; k2 < 3; ++k2) {
             d[k2] -= L[k2] * floor(d[k2] / L[k2] + 0.5);
@@ -121,6 +124,9 @@ __global__ void __launch_bounds__(256) k_set_state(const DevParams P, SortedStat
     }
     p.x = x[0]; p.y = x[1]; p.z = x[2];
     st.pos[i] = p;
+    float4 l = st.lo[i];
+    l.x = l.y = l.z = 0.f;
+    st.lo[i] = l;
   }
   if (vel || conc) {
     float4 v = st.vel[i];

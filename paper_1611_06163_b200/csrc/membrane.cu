@@ -17,7 +17,14 @@ __device__ __forceinline__ V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b
 __device__ __forceinline__ V3 cross3(V3 a, V3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
 __device__ __forceinline__ float dot3(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
 
-__device__ __forceinline__ float min_image(float d, float L) { return d - L * rintf(d / L); }
+// minimum-image difference a - b of two wrapped coordinates, exact where fp32 allows: the operand near L is
+// shifted by -L first (exact by Sterbenz), never the small one by +L
+__device__ __forceinline__ float min_image_diff(float a, float b, float L) {
+  float d = a - b;
+  if (d > 0.5f * L) d = (a - L) - b;
+  else if (d < -0.5f * L) d = a - (b - L);
+  return d;
+}
 
 // dU_WLC/dh = (kBT/p) (1/(4(1-x)^2) - 1/4 + x)   (from Eq 13)
 __device__ __forceinline__ float wlc_force(float kBT_over_p, float x) {
@@ -39,11 +46,14 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
   // ---- stage vertices (gather through slot_of_id)
   const uint32_t slot0 = A.slot_of_id[R.first_id];
   const float4 p0 = A.st.pos[slot0];
+  const float4 l0 = A.st.lo[slot0];
   for (int v = t; v < nv; v += NT) {
     uint32_t slot = A.slot_of_id[R.first_id + v];
     float4 p = A.st.pos[slot];
+    float4 l = A.st.lo[slot];
     float4 w = A.st.vel[slot];
-    sr[v] = {min_image(p.x - p0.x, P.box[0]), min_image(p.y - p0.y, P.box[1]), min_image(p.z - p0.z, P.box[2])};
+    sr[v] = {min_image_diff(p.x, p0.x, P.box[0]) + (l.x - l0.x), min_image_diff(p.y, p0.y, P.box[1]) + (l.y - l0.y),
+             min_image_diff(p.z, p0.z, P.box[2]) + (l.z - l0.z)};
     sv[v] = {w.x, w.y, w.z};
   }
   __syncthreads();

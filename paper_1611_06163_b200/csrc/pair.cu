@@ -197,10 +197,11 @@ __global__ void __launch_bounds__(256) k_pair(const __grid_constant__ DevParams 
     float sx = s_shift[h][0], sy = s_shift[h][1], sz = s_shift[h][2];
     for (int k = lane; k < cnt; k += 32) {
       float4 p = A.st.pos[s0 + k];
-      p.x -= sx; p.y -= sy; p.z -= sz;
+      float4 l = A.st.lo[s0 + k];
+      p.x = (p.x - sx) + l.x; p.y = (p.y - sy) + l.y; p.z = (p.z - sz) + l.z;
       sm.spos[d0 + k] = p;
       sm.svel[d0 + k] = A.st.vel[s0 + k];
-      sm.smeta[d0 + k] = A.st.meta[s0 + k];
+      sm.smeta[d0 + k] = __float_as_uint(l.w);
 #pragma unroll
       for (int s = 1; s < S; ++s) sm.scx[(s - 1) * hcap + d0 + k] = A.st.cx[(int64_t)(s - 1) * n + s0 + k];
     }
