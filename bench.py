@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the tDPD + RBC hot path (all rows of SURVEY.md §8(a)) on B200, one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A "step" is one velocity-Verlet step of the whole system through `tdpd_step`: wrap + cell hash, stable radix sort,
+cell table + reorder, non-bonded pair kernel, membrane kernel (second stream), fused integrator.
+Default workload: BASELINE.json config 5 (128^3 box, 6.29 M solvent particles + 1000 RBCs, two species), the
+configuration BASELINE.json names "for peak throughput and ncu roofline capture"; its state (>300 MB) is larger than
+the 126 MB L2, so no flush is needed between steps.  Smaller configs (--config 1..4) are timed step by step with an
+L2 flush (a 256 MB write) between steps.
+
+  value        particle-steps/s, device-timed (CUDA events on the library's pair stream), state resident in HBM
+  e2e          the same metric through the C ABI with HOST buffers: every step copies the whole state host->device
+               (tdpd_set_state, pinned memory), advances one step and reads it back (tdpd_get_state)
+  roofline     the pair kernel (dominant): algorithmic FLOPs of one launch (per-unit budget x the
+               exact pair census of the workload) / its CUDA-event duration, against the FP32 peak of DESIGN.md §7
+  cpu_baseline the fp64 oracle (oracle/, as it stands) on this box's host cores on a bounded sample of the workload
+
+--impl reference times the oracle alone (there is no reference implementation; the paper ships no code).
+Multi-GPU: "replicas only": each rank runs an independent replica, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import tdpd_workloads as W  # noqa: E402  (inputs only)
+
+L2_BYTES = 126 * 1024 * 1024
+SM_COUNT, LANES_PER_SM, SM_MAX_MHZ = 148, 128, 1965.0
+# FP32 peak of the plain ALUs: 148 SMs x 128 lanes x 2 FLOP (FMA) x 1.965 GHz
+FP32_PEAK_TFLOPS = SM_COUNT * LANES_PER_SM * 2 * SM_MAX_MHZ * 1e6 / 1e12
+# per-unit algorithmic budget, SURVEY.md §8(d) / DESIGN.md §7: (FLOP with FMA = 2, FP32+INT lane-instructions)
+OPS = dict(cand=(8, 7), flux=(8, 7), rflux=(9, 8), force=(28, 21), philox=(0, 70), boxmuller=(10, 18))
+
+
+# --------------------------------------------------------------------------------------------------------------
+def workload(c: int, rank: int = 0):
+    w = W.config(c)
+    if rank:  # replicas differ only in the random stream
+        w.params = dict(w.params, seed=int(w.params["seed"]) + 7919 * rank)
+    return w
+
+
+def sample_workload(c: int):
+    """Bounded sample of config c for the oracle leg: the same recipe, density, parameters and species on a smaller
+    box (configs 1-3 are used whole; 4-5 keep the RBC lattice spacing of the full box)."""
+    if c in (1, 2, 3):
+        return W.config(c), f"config{c}, whole system"
+    seed = W.BASE_SEED + c
+    rng = np.random.Generator(np.random.PCG64(seed + 1000))
+    from tdpd_workloads import mesh as _mesh
+    if c == 4:
+        box, grid = (25.6, 25.6, 32.0), (2, 2, 2)
+        ctr = W.lattice_centers(box, grid)
+    else:
+        box, grid = (25.6, 25.6, 25.6), (2, 2, 2)
+        ctr = W.lattice_centers(box, grid, rng, jitter=2.0)
+    w = W.make_suspension(f"config{c}-sample", box, 3.0, seed, ctr, _mesh.random_rotations(rng, len(ctr)),
+                          n_species=2)
+    return w, (f"config{c} recipe on a {box[0]}x{box[1]}x{box[2]} box: {w.n_solvent} solvent + {len(ctr)} RBCs "
+               f"(same density, lattice spacing, species and parameters)")
+
+
+def census(sim, w) -> dict:
+    """Exact pair census of the workload at the current positions (directed pairs): candidates of the 27-cell
+    stencil from the cell occupancy, pairs within r_c / r_cc from the library's integer census (both parity-tested
+    bit-exact against the oracle in tests/test_gpu_parity.py).  Setup only, never timed."""
+    b = sim.debug_binning()
+    nc = b["ncell"]
+    cnt = b["cell_count"].reshape(nc[2], nc[1], nc[0]).astype(np.int64)
+    nb = np.zeros_like(cnt)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                nb += np.roll(cnt, (dz, dy, dx), axis=(0, 1, 2))
+    cs = sim.debug_neighbor_census()
+    return dict(n_cand=int((cnt * nb).sum() - cnt.sum()), n_cc=int(cs["n_rcc"].sum()), n_c=int(cs["n_rc"].sum()),
+                cells=[int(x) for x in nc])
+
+
+def pair_budget(cen: dict, params: dict) -> dict:
+    """Algorithmic work of ONE pair-kernel launch."""
+    S = int(params["n_species"])
+    rf = bool(np.any(np.asarray(params["m_s"])[:S] != 0))
+    n_cand, n_cc, n_c = cen["n_cand"], cen["n_cc"], cen["n_c"]
+    r_c, r_cc = float(params["r_c"]), float(params["r_cc"])
+    n_any = max(n_cc, n_c) if r_cc >= r_c else n_c  # pairs that need at least one Gaussian
+    n_rng = n_any if rf else n_c
+    n_bm = (n_c if not rf else n_cc * ((S + 1 + 1) // 2)) if r_cc >= r_c else n_c  # Box-Muller calls (2 Gaussians)
+    n_philox = n_rng * (2 if (rf and S >= 3) else 1)
+    tot = [0, 0]
+    for k, cnt in (("cand", n_cand), ("flux", n_cc * S), ("rflux", n_cc * S if rf else 0), ("force", n_c),
+                   ("philox", n_philox), ("boxmuller", n_bm)):
+        tot[0] += OPS[k][0] * cnt
+        tot[1] += OPS[k][1] * cnt
+    return dict(flop=tot[0], lane_instr=tot[1])
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, r[3:7]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(nme)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                    samples=len(sm), reasons=sorted(reasons))
+
+
+# --------------------------------------------------------------------------------------------------------------
+def run_reference(args) -> dict:
+    """The oracle, as it stands, on the host cores (the tier's stand-in for a reference implementation)."""
+    import oracle
+    oracle.build()
+    w, what = sample_workload(args.config)
+    o = oracle.Oracle.from_workload(w)
+    o.compute_forces(0)
+    # bound the run: a step costs about the same as the force evaluation just timed
+    t0 = time.perf_counter(); o.step(1); t_step = time.perf_counter() - t0
+    budget = 150.0
+    steps = max(1, min(args.steps, int(budget / max(t_step, 1e-9))))
+    warm = max(0, min(args.warmup, int(0.2 * budget / max(t_step, 1e-9)) - 1))
+    if warm:
+        o.step(warm)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    v = w.n_total * steps / dt
+    cores = oracle.num_threads()
+    return {
+        "impl": "reference", "metric": "tDPD particle-steps/sec", "value": v, "unit": "particle-steps/s",
+        "n_gpus": args.gpus, "steps": steps, "warmup": warm + 1, "ms_per_step": 1e3 * dt / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config{args.config}", "sample": what, "n_particles": w.n_total},
+        "cpu_baseline": {"value": v, "unit": "particle-steps/s", "cores": cores, "kind": "oracle", "sample": what},
+        "e2e": {"value": v, "unit": "particle-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+def cpu_baseline(c: int, seconds: float = 20.0) -> dict:
+    import oracle
+    oracle.build()
+    w, what = sample_workload(c)
+    o = oracle.Oracle.from_workload(w)
+    t0 = time.perf_counter(); o.compute_forces(0); t_f = time.perf_counter() - t0
+    steps = max(1, min(200, int(seconds / max(t_f, 1e-9))))
+    t0 = time.perf_counter(); o.step(steps); dt = time.perf_counter() - t0
+    return {"value": w.n_total * steps / dt, "unit": "particle-steps/s", "cores": oracle.num_threads(),
+            "kind": "oracle", "sample": f"{what}; {steps} steps, {dt:.1f} s"}
+
+
+# --------------------------------------------------------------------------------------------------------------
+def run_ours(args) -> dict | None:
+    import torch
+    import paper_1611_06163_b200 as T
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    T.load_library()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+
+    c = args.config
+    w = workload(c, rank)
+    sim = T.Simulation.from_workload(w, device=local)
+    n, S = sim.n, sim.ns
+    K, Wm = args.steps, max(3, args.warmup)
+    state_bytes = n * (16 * 3 + 4 * max(S - 1, 0))
+    flush = state_bytes < 2 * L2_BYTES
+    stream = sim.stream_pair
+    flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=f"cuda:{local}") if flush else None
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sim.step(Wm)
+    sim.sync()
+    cen = census(sim, w)
+    bud = pair_budget(cen, w.params)
+
+    # ---- device-timed region: K steps, per-kernel-class events on the launching streams
+    sim.set_timing(True)
+    barrier()
+    clocks = ClockSampler(local) if rank == 0 else None
+    l0 = sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if not flush:
+        e0.record(stream)
+        sim.step(K)
+        e1.record(stream)
+        sim.sync()
+        ms = e0.elapsed_time(e1)
+    else:
+        evs = []
+        for _ in range(K):
+            with torch.cuda.stream(stream):
+                flush_buf.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            sim.step(1)
+            b.record(stream)
+            evs.append((a, b))
+        sim.sync()
+        ms = sum(a.elapsed_time(b) for a, b in evs)
+    launches = sim.launch_count - l0
+    barrier()
+    clk = clocks.stop() if clocks else None
+    tim = sim.get_timing()
+    sim.set_timing(False)
+
+    # ---- end to end through the C ABI with host buffers (pinned), every step: H2D state, one step, D2H state
+    Ke = max(3, min(K, 10))
+    pin = lambda wdt: torch.empty((n, wdt), dtype=torch.float32, pin_memory=True).numpy()
+    hb = dict(pos=pin(3), vel=pin(3), conc=pin(S))
+    sim.get_state(forces=False, out=hb)
+    for _ in range(2):
+        sim.set_state(hb["pos"], hb["vel"], hb["conc"]); sim.step(1); sim.get_state(forces=False, out=hb)
+    barrier()
+    t0 = time.perf_counter()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(Ke):
+        sim.set_state(hb["pos"], hb["vel"], hb["conc"])
+        sim.step(1)
+        sim.get_state(forces=False, out=hb)
+    b.record(stream)
+    sim.sync()
+    ms_e2e = max(a.elapsed_time(b), 1e3 * (time.perf_counter() - t0))
+    barrier()
+
+    tmax, temax, ntot = ms, ms_e2e, float(n)
+    if dist is not None:
+        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tmax, temax = float(t[0]), float(t[1])
+        t = torch.tensor([float(n)], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        ntot = float(t[0])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return None
+
+    # ---- roofline of the pair kernel (dominant)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak, hbm_src = (peaks["hbm_gbs"], "measured") if "hbm_gbs" in peaks else (6650.0, "fallback")
+    pair_ms = tim["pair"]["ms"] / max(tim["pair"]["launches"], 1)
+    ach = bud["flop"] / (pair_ms * 1e-3) / 1e12
+    issue_peak = SM_COUNT * LANES_PER_SM * SM_MAX_MHZ * 1e6  # lane-instructions / s
+    kernel_ms = {k: v["ms"] / max(K, 1) for k, v in tim.items()}
+    step_ms_sum = sum(kernel_ms.values())
+    pair_hbm_bytes = n * (32 + 16 + 16 + 8 * max(S - 1, 0))  # pos+vel (+lo, meta) in, F4 (+Qx) out, per particle
+    roof = {
+        "kernel": "k_pair", "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+        "frac": ach / FP32_PEAK_TFLOPS,
+        "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md §7); not in MEASURED_PEAKS.json",
+        "traffic": None,
+        "ms_per_launch": pair_ms, "flop_per_launch": bud["flop"], "share_of_step": kernel_ms["pair"] / step_ms_sum,
+        "issue_slot_frac": bud["lane_instr"] / (pair_ms * 1e-3) / issue_peak,
+        "hbm_gbs_algorithmic": pair_hbm_bytes / (pair_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
+        "hbm_peak_source": hbm_src, "census": cen,
+    }
+    out = {
+        "metric": "tDPD particle-steps/sec", "value": ntot * K / (tmax * 1e-3), "unit": "particle-steps/s",
+        "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": tmax / K, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config{c}", "n_particles": n, "n_rbc": sim.n_rbc, "n_species": S,
+                   "box": [float(x) for x in w.params["box"]], "random_flux": bool(np.any(w.params["m_s"][:S] != 0)),
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": ("256 MB flush write between timed steps" if flush else
+                          f"no flush: state {state_bytes / 2**20:.0f} MB per side > 126 MB L2")},
+        "e2e": {"value": ntot * Ke / (temax * 1e-3), "unit": "particle-steps/s", "steps": Ke,
+                "h2d_bytes_per_step": int(n * (6 + S) * 4), "d2h_bytes_per_step": int(n * (6 + S) * 4),
+                "what": "per step: tdpd_set_state (pinned host -> device), tdpd_step(1) incl. the force "
+                        "re-evaluation set_state implies, tdpd_get_state (device -> pinned host)"},
+        "gpu_launches": int(launches), "clocks": clk, "roofline": roof,
+        "kernel_ms_per_step": kernel_ms,
+    }
+    if not args.no_cpu:
+        out["cpu_baseline"] = cpu_baseline(c)
+    if dist is not None:
+        dist.destroy_process_group()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        print(json.dumps(run_reference(args)), flush=True)
+        return
+    out = run_ours(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()
