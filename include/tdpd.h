@@ -181,10 +181,11 @@ int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], double ms[TDPD
 /* Number of kernels the library launched since creation (bench.py's gpu_launches). */
 int64_t tdpd_launch_count(const tdpd_sim* s);
 
-/* Pair-kernel configuration knobs (tuning; results are identical up to fp32 summation order within a cell):
- * brick_log2 in 3..5 = cells per CTA brick (2x2x2, 4x2x2, 4x4x2); 0 = automatic.  use_graph: capture the
- * step into a CUDA graph. */
-int tdpd_set_tuning(tdpd_sim* s, int32_t brick_log2, int32_t use_graph);
+/* Pair-kernel launch knobs (tuning; results are identical up to the fp32 summation order of a particle's
+ * neighbours): pair_threads in {32, 64, 128, 256} = particles per CTA, list_cap in 4..400 = entries of the
+ * per-thread neighbour list in shared memory (a full list is evaluated early, never overflowed); 0 = automatic.
+ * ESTATE after tdpd_set_workspace. */
+int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap);
 
 const char* tdpd_last_error(const tdpd_sim* s);
 int tdpd_destroy(tdpd_sim* s);

@@ -134,7 +134,7 @@ def _f32(a):
 class Simulation:
     """One tDPD + RBC simulation on one GPU.  Methods mirror the C ABI one to one."""
 
-    def __init__(self, params: dict, device: int = 0, brick_log2: int = 0):
+    def __init__(self, params: dict, device: int = 0, pair_threads: int = 0, list_cap: int = 0):
         import torch
 
         self.L = load_library()
@@ -156,8 +156,8 @@ class Simulation:
         self.h = h
         self.workspace = None
         self._ntri = []
-        if brick_log2:
-            self._ck(self.L.tdpd_set_tuning(self.h, brick_log2, 0))
+        if pair_threads or list_cap:
+            self._ck(self.L.tdpd_set_tuning(self.h, pair_threads, list_cap))
 
     def _ck(self, rc):
         if rc != OK:

@@ -54,8 +54,9 @@ struct tdpd_sim {
   uint32_t ncells = 0;
   int key_bits = 0;
   std::vector<uint32_t> cell_rank, rank_cell;
-  std::vector<Brick> bricks;
-  int brick_log2 = 0, tune_brick = 0, bx = 0, by = 0, bz = 0, pair_nt = 128, hcap = 0, lcap = 0;
+  int pair_nt = 256, lcap = 72, tune_nt = 0, tune_lcap = 0;
+  PairRec rec = {nullptr, nullptr, nullptr};
+  uint32_t* keys_sorted = nullptr;
   int mem_nchunk = 1, mem_nt = 256, max_nv = 0;
   // device
   void* ws = nullptr;
@@ -66,7 +67,6 @@ struct tdpd_sim {
   uint32_t *keys[2] = {nullptr, nullptr}, *vals[2] = {nullptr, nullptr};
   void* sort_scratch = nullptr;
   uint32_t *cell_start = nullptr, *cell_rank_d = nullptr, *rank_cell_d = nullptr, *slot_of_id = nullptr;
-  Brick* bricks_d = nullptr;
   float4 *F4 = nullptr, *Fb = nullptr;
   float *Qx = nullptr, *staging = nullptr;
   int* err_d = nullptr;
@@ -130,6 +130,13 @@ void derive_params(const tdpd_params& p, DevParams& d) {
     d.ncell[a] = (int)std::floor((double)p.box[a] / rcut);
     d.cell_inv[a] = (float)((double)d.ncell[a] / (double)p.box[a]);
     d.cell_edge[a] = (float)((double)p.box[a] / (double)d.ncell[a]);
+    {  // edge_q: the cell edge truncated to 13 significant bits, so that c * edge_q is exact in fp32 for c < 1024
+      int ex;
+      double mant = std::frexp((double)p.box[a] / (double)d.ncell[a], &ex);
+      double eq = std::ldexp(std::floor(mant * 8192.0) / 8192.0, ex);
+      d.edge_q[a] = (float)eq;
+      d.gap[a] = (float)((double)p.box[a] - (double)d.ncell[a] * eq);
+    }
     d.body[a] = p.body_force[a];
   }
   d.half_box_z = 0.5f * p.box[2];
@@ -353,7 +360,7 @@ extern "C" int tdpd_add_rbc_mesh(tdpd_sim* s, int32_t nv, const float* verts, co
 }
 
 // =====================================================================================================
-// grid, bricks, launch configuration
+// grid, launch configuration
 // =====================================================================================================
 static void build_grid(tdpd_sim* s) {
   const int* nc = s->dp.ncell;
@@ -375,35 +382,15 @@ static void build_grid(tdpd_sim* s) {
     uint32_t x = lin % nc[0], y = (lin / nc[0]) % nc[1], z = lin / (nc[0] * nc[1]);
     s->rank_cell[r] = x | (y << 10) | (z << 20);
   }
-  // launch configuration of the pair kernel
-  double mpc = (double)s->n / (double)s->ncells;  // mean particles per cell
-  int S = s->prm.n_species;
-  int k = s->tune_brick ? s->tune_brick : ((double)s->ncells / 16.0 >= 2.0 * 148 ? 4 : 3);
-  for (;; --k) {
-    s->bx = 1 << ((k + 2) / 3); s->by = 1 << ((k + 1) / 3); s->bz = 1 << (k / 3);
-    double mb = mpc * (1 << k);
-    int nt = (int)(mb + 3.0 * std::sqrt(mb + 1.0) + 31) / 32 * 32;
-    s->pair_nt = std::min(256, std::max(64, nt));
-    double mh = mpc * (s->bx + 2) * (s->by + 2) * (s->bz + 2);
-    s->hcap = ((int)(mh + 8.0 * std::sqrt(mh + 1.0)) + (s->rbcs.empty() ? 32 : 384) + 31) / 32 * 32;
+  // launch configuration of the pair kernel: NT consecutive slots per CTA; small systems use smaller CTAs so that
+  // every SM gets several; the two-ended hit list holds ~1.3 x the mean number of neighbours inside the cutoff
+  {
     double rcut = std::max(s->prm.r_c, s->prm.r_cc);
-    double cellvol = (double)s->dp.cell_edge[0] * s->dp.cell_edge[1] * s->dp.cell_edge[2];
-    double mn = 4.18879 * rcut * rcut * rcut * mpc / cellvol;  // mean neighbours within the cutoff
-    s->lcap = std::min(512, ((int)(mn * 1.3) + 16 + 1) / 2 * 2);
-    size_t smem = td_pair_smem_bytes(S, s->bx, s->by, s->bz, s->hcap, s->lcap, s->pair_nt);
-    if ((smem <= 200 * 1024 && s->hcap <= 65535) || k == 3) break;
-  }
-  s->brick_log2 = k;
-  s->bricks.clear();
-  uint32_t r = 0;
-  while (r < s->ncells) {
-    uint32_t code = codes[r].first >> k, r1 = r;
-    while (r1 < s->ncells && (codes[r1].first >> k) == code) ++r1;
-    uint32_t base = code << k;  // decode origin
-    int o[3] = {0, 0, 0};
-    for (int b = 0; b < 30; ++b) o[b % 3] |= (int)((base >> b) & 1u) << (b / 3);
-    s->bricks.push_back(Brick{o[0], o[1], o[2], r, r1 - r});
-    r = r1;
+    double mn = 4.18879 * rcut * rcut * rcut * (double)s->n / ((double)s->prm.box[0] * s->prm.box[1] * s->prm.box[2]);
+    int lc = ((int)(mn * 1.2) + 6 + 1) / 2 * 2;
+    s->lcap = s->tune_lcap ? s->tune_lcap : std::min(160, std::max(16, lc));
+    int nt = s->n >= 148 * 8 * 256 ? 256 : (s->n >= 148 * 8 * 128 ? 128 : 64);
+    s->pair_nt = s->tune_nt ? s->tune_nt : nt;
   }
   // membrane kernel: CTAs per membrane so that small suspensions still fill the machine
   int M = (int)s->rbcs.size();
@@ -443,7 +430,9 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->cell_start = c.take<uint32_t>(s->ncells + 1);
   s->cell_rank_d = c.take<uint32_t>(s->ncells);
   s->rank_cell_d = c.take<uint32_t>(s->ncells);
-  s->bricks_d = c.take<Brick>(s->bricks.size());
+  s->rec.P4 = c.take<float4>(n);
+  s->rec.X4 = c.take<float4>(n);
+  s->rec.Y2 = c.take<float2>(S > 2 ? n : 1);
   s->slot_of_id = c.take<uint32_t>(n);
   s->F4 = c.take<float4>(n);
   s->Fb = c.take<float4>(n);
@@ -521,7 +510,6 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
   }
   CK(cudaMemcpyAsync(s->cell_rank_d, s->cell_rank.data(), s->ncells * 4, cudaMemcpyHostToDevice, q));
   CK(cudaMemcpyAsync(s->rank_cell_d, s->rank_cell.data(), s->ncells * 4, cudaMemcpyHostToDevice, q));
-  CK(cudaMemcpyAsync(s->bricks_d, s->bricks.data(), s->bricks.size() * sizeof(Brick), cudaMemcpyHostToDevice, q));
   // membranes
   std::vector<MeshTemplateDev> td(s->tmpls.size());
   std::vector<unsigned char> topo;
@@ -611,8 +599,9 @@ int bin_and_sort(tdpd_sim* s, int mode /*0 keys only, 1 open, 2 close+open*/) {
   }
   {
     Scope t(s, 2, s->sA);
-    td_launch_reorder(s->st[c], s->st[c ^ 1], s->keys[side], s->vals[side], s->n, s->prm.n_species, s->ncells,
-                      s->cell_start, s->slot_of_id, s->sA);
+    td_launch_reorder(s->dp, s->st[c], s->st[c ^ 1], s->rec, s->keys[side], s->vals[side], s->rank_cell_d, s->n,
+                      s->ncells, s->cell_start, s->slot_of_id, s->sA);
+    s->keys_sorted = s->keys[side];
     s->launches += 1; s->timers[2].launches += 1;
   }
   s->cur = c ^ 1;
@@ -631,10 +620,10 @@ int eval_forces(tdpd_sim* s) {
   {
     Scope t(s, 3, s->sA);
     PairArgs A;
-    A.st = s->st[c]; A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
-    A.bricks = s->bricks_d; A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step = (uint32_t)s->step;
-    A.bx = s->bx; A.by = s->by; A.bz = s->bz; A.hcap = s->hcap; A.lcap = s->lcap; A.err = s->err_d;
-    int rc = td_launch_pair(s->dp, A, (int)s->bricks.size(), s->pair_nt, s->sA);
+    A.rec = s->rec; A.vel = s->st[c].vel; A.keys = s->keys_sorted;
+    A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
+    A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step = (uint32_t)s->step; A.lcap = s->lcap; A.err = s->err_d;
+    int rc = td_launch_pair(s->dp, A, s->pair_nt, s->sA);
     if (rc) return fail(s, TDPD_ECUDA, std::string("pair kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
     s->launches += 1; s->timers[3].launches += 1;
   }
@@ -661,7 +650,8 @@ int ensure_forces(tdpd_sim* s) {
   if (!s->finalized) return fail(s, TDPD_ESTATE, "tdpd_set_workspace has not been called");
   CK(cudaSetDevice(s->device));
   if (s->have_forces) return TDPD_OK;
-  if (!s->binned) { int rc = bin_and_sort(s, 0); if (rc) return rc; }
+  // always re-bin: the reorder kernel also refreshes the pair kernel's records (concentrations, positions)
+  { int rc = bin_and_sort(s, 0); if (rc) return rc; }
   return eval_forces(s);
 }
 }  // namespace
@@ -706,7 +696,7 @@ static int check_err_word(tdpd_sim* s) {
     int zero = 0;
     cudaMemcpy(s->err_d, &zero, sizeof zero, cudaMemcpyHostToDevice);
     std::string m;
-    if (w & TD_ERR_HALO_OVERFLOW) m += "pair kernel: halo of a brick exceeds its shared-memory capacity; ";
+    if (w & TD_ERR_CELL_OVERFLOW) m += "pair kernel: a cell holds more than 2047 particles; ";
     if (w & TD_ERR_NONFINITE) m += "non-finite value in the state; ";
     if (w & TD_ERR_BOND_OVERSTRETCH) m += "a WLC bond reached x >= 1; ";
     return fail(s, TDPD_EUNSTABLE, m);
@@ -929,12 +919,14 @@ extern "C" int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], dou
 
 extern "C" int64_t tdpd_launch_count(const tdpd_sim* s) { return s ? s->launches : 0; }
 
-extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t brick_log2, int32_t use_graph) {
+extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap) {
   if (!s) return TDPD_EINVAL;
-  (void)use_graph;
   if (s->finalized) return fail(s, TDPD_ESTATE, "tuning must be set before tdpd_set_workspace");
-  if (brick_log2 != 0 && (brick_log2 < 3 || brick_log2 > 5)) return fail(s, TDPD_EINVAL, "brick_log2 must be 0 or 3..5");
-  s->tune_brick = brick_log2;
+  if (pair_threads != 0 && pair_threads != 32 && pair_threads != 64 && pair_threads != 128 && pair_threads != 256)
+    return fail(s, TDPD_EINVAL, "pair_threads must be 0, 32, 64, 128 or 256");
+  if (list_cap != 0 && (list_cap < 4 || list_cap > 400)) return fail(s, TDPD_EINVAL, "list_cap must be 0 or 4..400");
+  s->tune_nt = pair_threads;
+  s->tune_lcap = list_cap;
   return TDPD_OK;
 }
 

@@ -121,10 +121,13 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
   }
 }
 
-// gather the state into the new order, record slot_of_id for membrane vertices, fill the cell-start table
+// gather the state into the new order, record slot_of_id for membrane vertices, fill the cell-start table and
+// write the pair kernel's records: position relative to the cell origin o_c = c * edge_q (exact product; the
+// subtraction hi - o_c is exact too, so rel carries the full two-float position to ~2^-24), id, concentrations, meta
 template <int S>
-__global__ void __launch_bounds__(256) k_reorder(SortedState src, SortedState dst, const uint32_t* __restrict__ keys,
-                                                 const uint32_t* __restrict__ vals, int64_t n, uint32_t ncell,
+__global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState src, SortedState dst, PairRec rec,
+                                                 const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
+                                                 const uint32_t* __restrict__ rank_cell, int64_t n, uint32_t ncell,
                                                  uint32_t* __restrict__ cell_start, uint32_t* __restrict__ slot_of_id) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -137,8 +140,19 @@ __global__ void __launch_bounds__(256) k_reorder(SortedState src, SortedState ds
   dst.pos[i] = p;
   dst.vel[i] = v;
   dst.lo[i] = l;
+  float cxv[3] = {0.f, 0.f, 0.f};
 #pragma unroll
-  for (int s = 1; s < S; ++s) dst.cx[(int64_t)(s - 1) * n + i] = src.cx[(int64_t)(s - 1) * n + from];
+  for (int s = 1; s < S; ++s) {
+    cxv[s - 1] = src.cx[(int64_t)(s - 1) * n + from];
+    dst.cx[(int64_t)(s - 1) * n + i] = cxv[s - 1];
+  }
+  const uint32_t pc = __ldg(&rank_cell[k]);
+  const float ox = (float)(pc & 1023u) * P.edge_q[0], oy = (float)((pc >> 10) & 1023u) * P.edge_q[1],
+              oz = (float)(pc >> 20) * P.edge_q[2];
+  rec.P4[i] = make_float4(__fadd_rn(__fsub_rn(p.x, ox), l.x), __fadd_rn(__fsub_rn(p.y, oy), l.y),
+                          __fadd_rn(__fsub_rn(p.z, oz), l.z), p.w);
+  rec.X4[i] = make_float4(v.w, cxv[0], l.w, 0.0f);
+  if (S > 2) rec.Y2[i] = make_float2(cxv[1], cxv[2]);
   if (m >> 2) slot_of_id[__float_as_uint(p.w)] = (uint32_t)i;
   // cell_start[r] = first slot whose key >= r
   uint32_t kprev = i == 0 ? 0u : keys[i - 1] + 1u;
@@ -176,15 +190,15 @@ int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits
   return side;
 }
 
-void td_launch_reorder(const SortedState& src, const SortedState& dst, const uint32_t* keys, const uint32_t* vals,
-                       int64_t n, int n_species, uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id,
-                       cudaStream_t st) {
+void td_launch_reorder(const DevParams& P, const SortedState& src, const SortedState& dst, const PairRec& rec,
+                       const uint32_t* keys, const uint32_t* vals, const uint32_t* rank_cell, int64_t n,
+                       uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
-  switch (n_species) {
-    case 1: k_reorder<1><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
-    case 2: k_reorder<2><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
-    case 3: k_reorder<3><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
-    default: k_reorder<4><<<nb, 256, 0, st>>>(src, dst, keys, vals, n, ncell, cell_start, slot_of_id); break;
+  switch (P.n_species) {
+    case 1: k_reorder<1><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
+    case 2: k_reorder<2><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
+    case 3: k_reorder<3><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
+    default: k_reorder<4><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
   }
 }

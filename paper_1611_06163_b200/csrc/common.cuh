@@ -15,6 +15,10 @@ struct DevParams {
   int ncell[3];
   float cell_inv[3];   // (float)(n_a / L_a): binning multiplier (R-bin)
   float cell_edge[3];  // L_a / n_a
+  // pair-kernel coordinates are stored RELATIVE to a per-cell origin o_c = c * edge_q (exact in fp32: edge_q keeps
+  // 13 significant bits and c < 1024), so that differences between neighbouring cells are exact; gap = L - n edge_q
+  // is the extra displacement across the periodic boundary
+  float edge_q[3], gap[3];
   float r_c, r_cc, rc2, rcc2, rcut2, inv_rc, inv_rcc;
   float dt, half_dt;
   // type-pair tables, index ti*TD_T + tj
@@ -55,8 +59,19 @@ __device__ __forceinline__ void td_philox(uint32_t c0, uint32_t c1, uint32_t c2,
 }
 
 // word -> uniform strictly inside (0,1): u = ((x >> 9) + 1/2) 2^-23 (exact in fp32)
+// evaluated without an int->float conversion: 1.m - (1 - 2^-24) with m = x >> 9 is exact (Sterbenz + 24-bit result)
 __device__ __forceinline__ float td_uniform(uint32_t x) {
-  return fmaf((float)(x >> 9), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
+  return __uint_as_float((x >> 9) | 0x3f800000u) - 0.99999994039535522f;
+}
+__device__ __forceinline__ float td_sqrt_approx(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float td_rsqrt_approx(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 // Box-Muller: R = sqrt(-2 ln ua); (g_cos, g_sin) = R (cos 2 pi ub, sin 2 pi ub).
@@ -66,12 +81,12 @@ __device__ __forceinline__ void td_box_muller(uint32_t xa, uint32_t xb, float& g
   float q;
   if (xa >= 0xFFFF8000u) {
     // t = 1 - ua = ((2^23 - 1 - (xa >> 9)) + 1/2) 2^-23, exact
-    float t = fmaf((float)(8388607u - (xa >> 9)), 1.1920928955078125e-07f, 5.9604644775390625e-08f);
+    float t = fmaf((float)(8388607u - (xa >> 9)), 1.1920928955078125e-07f, 5.9604644775390625e-08f);  // rare
     q = fmaf(t, t, 2.0f * t);
   } else {
     q = -1.3862943611198906f * __log2f(td_uniform(xa));  // -2 ln 2 * lg2(u)
   }
-  float R = sqrtf(q);
+  float R = td_sqrt_approx(q);
   float ang = 6.283185307179586f * td_uniform(xb);
   g_cos = R * __cosf(ang);
   g_sin = R * __sinf(ang);
@@ -85,23 +100,25 @@ struct SortedState {   // one side of the ping-pong, cell-sorted order
   float4* lo;      // low-order words of x, y, z (position = pos + lo, two-float), td_meta (bits)
 };
 
-struct Brick {  // one CTA of the pair kernel: 2^k consecutive Morton codes
-  int ox, oy, oz;       // cell coordinates of the brick origin
-  uint32_t r0, ncell;   // first Morton rank, number of existing cells
+// pair-kernel records, written by the reorder kernel in cell-sorted order (read-only in the pair kernel)
+struct PairRec {
+  float4* P4;   // x, y, z relative to the cell origin o_c (see DevParams::edge_q), id (bits)
+  float4* X4;   // C_0, C_1, td_meta (bits), 0
+  float2* Y2;   // C_2, C_3 (only when n_species > 2)
 };
 
 struct PairArgs {
-  SortedState st;
+  PairRec rec;
+  const float4* vel;           // vx, vy, vz, C_0 (SortedState::vel)
+  const uint32_t* keys;        // [n] Morton rank of the cell of each slot (sorted)
   const uint32_t* cell_start;  // [ncell + 1] by Morton rank
   const uint32_t* cell_rank;   // [ncell] x-fastest linear cell -> Morton rank
   const uint32_t* rank_cell;   // [ncell] Morton rank -> packed cx | cy << 10 | cz << 20
-  const Brick* bricks;
   float4* F4;                  // Fx, Fy, Fz, Q_0 by slot
   float* Qx;                   // [(S-1)][n]
   int64_t n;
   uint32_t step;               // RNG step word
-  int bx, by, bz;              // brick dims in cells
-  int hcap, lcap;              // smem capacities: halo particles, list entries per thread
+  int lcap;                    // list entries per thread
   int* err;                    // device error word
 };
 
@@ -142,7 +159,7 @@ struct MembraneArgs {
   int* err;
 };
 
-enum { TD_ERR_HALO_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4 };
+enum { TD_ERR_CELL_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4 };
 
 // ---- launchers (each .cu exposes host functions; all launches are asynchronous on `st`) -------------------
 void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
@@ -157,11 +174,11 @@ size_t td_sort_scratch_bytes(int64_t n);
 // sorts (keys, vals); result ends in keys[out_side]/vals[out_side]; returns out_side
 int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits, void* scratch, cudaStream_t st,
                    int* n_launches);
-void td_launch_reorder(const SortedState& src, const SortedState& dst, const uint32_t* keys, const uint32_t* vals,
-                       int64_t n, int n_species, uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id,
-                       cudaStream_t st);
-int td_launch_pair(const DevParams& P, const PairArgs& A, int nbricks, int nthreads, cudaStream_t st);
-size_t td_pair_smem_bytes(int n_species, int bx, int by, int bz, int hcap, int lcap, int nthreads);
+void td_launch_reorder(const DevParams& P, const SortedState& src, const SortedState& dst, const PairRec& rec,
+                       const uint32_t* keys, const uint32_t* vals, const uint32_t* rank_cell, int64_t n,
+                       uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, cudaStream_t st);
+int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st);
+size_t td_pair_smem_bytes(int lcap, int nthreads);
 int td_launch_membrane(const DevParams& P, const MembraneArgs& A, int n_rbc, int max_nv, int nthreads,
                        cudaStream_t st);
 void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, const float4* Fb, int64_t n,

@@ -4,29 +4,32 @@
 //                                                                                     r < r_cc  (Eq 7-10)
 // Every pair is evaluated on both sides; there are no atomics, so per-particle sums are deterministic.
 //
-// Design (B200): one CTA owns a brick of 2^k Morton-consecutive cells whose particles are contiguous in the sorted
-// order.  The brick's halo (brick +- 1 cell) is staged into shared memory in halo-local x-fastest order, in
-// coordinates RELATIVE to the brick origin (periodic images resolved at staging, so the inner loops have no
-// minimum-image arithmetic and fp32 differences are exact to ~2^-22).  One thread owns one particle:
-//   phase 1 scans the 9 x-runs (3 cells each, contiguous in shared memory) of its stencil and appends the indices of
-//           the candidates inside the cutoffs to a private two-ended list in shared memory (front: r < r_c, back:
-//           r_c <= r < r_cc), so that
-//   phase 2 runs the expensive per-pair work (Philox-4x32-10, Box-Muller, weights) over dense lists instead of
-//           under a 14 %-taken branch.
+// Design (B200).  One thread owns one particle of the cell-sorted order; a CTA owns NT consecutive slots, i.e. a
+// compact blob of ~NT/13 Morton-consecutive cells.  Nothing is staged: the candidate positions are read through
+// L1 (lanes of one cell read the same address), in coordinates RELATIVE to their cell origin (PairRec::P4), so
+// that the inner loops have no minimum-image arithmetic and fp32 differences are exact to ~2^-22 at any box size.
+//   prologue  the CTA builds, for each of its cells, the table of the 27 neighbour cells: first slot, particle
+//             count and the displacement of the neighbour's origin (periodic image resolved here).
+//   phase 1   each thread scans the 27 cells and appends the hits, branch-free, to a private two-ended list of
+//             16-bit entries (neighbour cell << 11 | offset) in shared memory: front r < min(r_c, r_cc), back the
+//             ring up to max(r_c, r_cc).  86 % of the candidates are rejected here for ~13 instructions each.
+//   phase 2   runs the expensive per-pair work (Philox-4x32-10, Box-Muller, weights) over the dense lists, two
+//             entries per iteration for instruction-level parallelism.
+// Shared memory per thread is ~210 B, so 32 warps per SM are resident (the first version staged whole halos and
+// ran 8).
 #include "common.cuh"
 
 namespace {
 
+constexpr int MAXLOC = 32;   // cells per table chunk
+constexpr int OFFBITS = 11;  // list entry: neighbour index (0..26) << 11 | offset inside the neighbour cell
+constexpr uint32_t OFFMASK = (1u << OFFBITS) - 1u;
+
 struct PairSmem {
-  int* hs;         // [NH + 1] exclusive prefix of halo-cell counts (halo-local x-fastest)
-  int* bcs;        // [NCB + 1] brick-cell prefix (Morton rank order) of the brick's own particles
-  int* bh;         // [NCB] halo-cell index of each brick cell
-  float4* spos;    // [hcap] x', y', z' relative to the brick origin, id bits
-  float4* svel;    // [hcap] vx, vy, vz, C_0
-  uint32_t* smeta; // [hcap]
-  float* scx;      // [(S-1)][hcap]
-  uint16_t* list;  // [lcap][NT]
-  float* tab;      // type-pair tables
+  float4* tso;      // [MAXLOC * 27] first slot (bits), displacement of the neighbour origin x, y, z
+  uint32_t* tcnt;   // [MAXLOC * 27] particles in the neighbour cell
+  float* tab;       // [8 * 16] type-pair tables: a, gamma, sigma/sqrt(dt), s_R, kappa[0..3]
+  uint16_t* list;   // [lcap][NT]
 };
 
 __device__ __forceinline__ float td_pow_w(float w, float s) {
@@ -34,58 +37,73 @@ __device__ __forceinline__ float td_pow_w(float w, float s) {
   return s == 0.0f ? 1.0f : exp2f(s * __log2f(fmaxf(w, 0.0f)));
 }
 
-template <int S, bool RANDFLUX, bool FASTW, bool FORCE>
-__device__ __forceinline__ void pair_eval(const DevParams& P, const PairSmem& sm, int hcap, int j, float xi_, float yi,
-                                          float zi, const float4& vi, const float* ci, uint32_t idi, uint32_t mi,
-                                          uint32_t step, float& fx, float& fy, float& fz, float* q) {
-  float4 pj = sm.spos[j];
-  float4 vj = sm.svel[j];
-  uint32_t mj = sm.smeta[j];
-  uint32_t idj = __float_as_uint(pj.w);
-  float dx = xi_ - pj.x, dy = yi - pj.y, dz = zi - pj.z;
-  float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-  float rinv = rsqrtf(r2);
-  float r = r2 * rinv;
-  bool excl = P.excl_same && (mi >> 2) != 0u && (mi >> 2) == (mj >> 2);  // R16
-  int tt = (int)(mi & 3u) * TD_T + (int)(mj & 3u);
+struct Self {  // the thread's own particle
+  float x, y, z;
+  float4 v;  // vx, vy, vz, C_0
+  float c[TD_S];
+  uint32_t id, meta;
+  int lc27;  // 27 * local cell index
+};
+
+// One list entry.  MODE 0: r < min(r_c, r_cc): force and flux; MODE 1: ring with r_cc > r_c: flux only;
+// MODE 2: ring with r_c > r_cc: force only.  wgt = 0 turns the entry into a no-op (odd tail of the unrolled loop).
+template <int S, bool RANDFLUX, bool FASTW, int MODE>
+__device__ __forceinline__ void pair_eval(const DevParams& P, const PairArgs& A, const PairSmem& sm, const Self& me,
+                                          uint32_t e, float wgt, float& fx, float& fy, float& fz, float* q) {
+  constexpr bool FORCE = MODE != 1, FLUX = MODE != 2;
+  const float4 te = sm.tso[me.lc27 + (int)(e >> OFFBITS)];
+  const uint32_t j = __float_as_uint(te.x) + (e & OFFMASK);
+  const float4 pj = __ldg(&A.rec.P4[j]);
+  const float4 xj = __ldg(&A.rec.X4[j]);
+  const uint32_t idj = __float_as_uint(pj.w), mj = __float_as_uint(xj.z);
+  const float dx = (me.x - te.y) - pj.x, dy = (me.y - te.z) - pj.y, dz = (me.z - te.w) - pj.z;
+  const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+  const float rinv = td_rsqrt_approx(fmaxf(r2, 1e-30f));
+  const float r = r2 * rinv;
+  const bool excl = P.excl_same && (me.meta >> 2) != 0u && (me.meta >> 2) == (mj >> 2);  // R16
+  const float keep = (excl || r2 < 1e-12f) ? 0.0f : wgt;                                  // R22
+  const int tt = (int)(me.meta & 3u) * TD_T + (int)(mj & 3u);
   float g0 = 0.f, g1 = 0.f, g2 = 0.f, g3 = 0.f, g4 = 0.f, g5 = 0.f;
-  if (RANDFLUX || FORCE) {
-    uint32_t lo = min(idi, idj), hi = max(idi, idj);
+  if (FORCE || RANDFLUX) {
+    const uint32_t lo = min(me.id, idj), hi = max(me.id, idj);
     uint32_t x0, x1, x2, x3;
-    td_philox(lo, hi, step, 0u, P.key0, P.key1, x0, x1, x2, x3);
+    td_philox(lo, hi, A.step, 0u, P.key0, P.key1, x0, x1, x2, x3);
     td_box_muller(x0, x1, g0, g1);
-    if (RANDFLUX && S >= 2) td_box_muller(x2, x3, g2, g3);
-    if (RANDFLUX && S >= 3) {
-      td_philox(lo, hi, step, 4u, P.key0, P.key1, x0, x1, x2, x3);
+    if (FLUX && RANDFLUX && S >= 2) td_box_muller(x2, x3, g2, g3);
+    if (FLUX && RANDFLUX && S >= 3) {
+      td_philox(lo, hi, A.step, 4u, P.key0, P.key1, x0, x1, x2, x3);
       td_box_muller(x0, x1, g4, g5);
     }
   }
-  float keep = excl ? 0.0f : 1.0f;
-  if (!FORCE || r2 < P.rcc2) {
-    float w = fmaxf(1.0f - r * P.inv_rcc, 0.0f);
-    float sgn = idi < idj ? keep : -keep;
+  if (FLUX) {
+    const float w = fmaxf(1.0f - r * P.inv_rcc, 0.0f);
+    const float sgn = me.id < idj ? keep : -keep;
 #pragma unroll
     for (int s = 0; s < S; ++s) {
-      float cj = s == 0 ? vj.w : sm.scx[(s - 1) * hcap + j];
-      float kap = sm.tab[(4 + s) * 16 + tt];
+      float cj;
+      if (s == 0) cj = xj.x;
+      else if (s == 1) cj = xj.y;
+      else { const float2 y = __ldg(&A.rec.Y2[j]); cj = s == 2 ? y.x : y.y; }
+      const float kap = sm.tab[(4 + s) * 16 + tt];
       float wdc, wrc;
       if (FASTW) { wdc = w * w; wrc = w; }
-      else { wdc = td_pow_w(w, P.s_c[s]); wrc = sqrtf(wdc); }
-      float qq = -kap * wdc * (ci[s] - cj) * keep;
+      else { wdc = td_pow_w(w, P.s_c[s]); wrc = td_sqrt_approx(wdc); }
+      float qq = -kap * wdc * (me.c[s] - cj) * keep;
       if (RANDFLUX) {
-        float zeta = s == 0 ? g1 : s == 1 ? g2 : s == 2 ? g4 : g5;
-        float csum = fmaxf(ci[s] + cj, 0.0f);
-        qq = fmaf(sgn * zeta * wrc, sqrtf(kap * csum * P.epsc[s]), qq);
+        const float zeta = s == 0 ? g1 : s == 1 ? g2 : s == 2 ? g4 : g5;
+        const float csum = fmaxf(me.c[s] + cj, 0.0f);
+        qq = fmaf(sgn * zeta * wrc, td_sqrt_approx(kap * csum * P.epsc[s]), qq);
       }
       q[s] += qq;
     }
   }
   if (FORCE) {
-    float wc = fmaxf(1.0f - r * P.inv_rc, 0.0f);
+    const float4 vj = __ldg(&A.vel[j]);
+    const float wc = fmaxf(1.0f - r * P.inv_rc, 0.0f);
     float wR, wD;
-    if (FASTW) { wR = sqrtf(wc); wD = wc; }
+    if (FASTW) { wR = td_sqrt_approx(wc); wD = wc; }
     else { wR = td_pow_w(wc, sm.tab[3 * 16 + tt]); wD = wR * wR; }
-    float edv = (dx * (vi.x - vj.x) + dy * (vi.y - vj.y) + dz * (vi.z - vj.z)) * rinv;
+    const float edv = (dx * (me.v.x - vj.x) + dy * (me.v.y - vj.y) + dz * (me.v.z - vj.z)) * rinv;
     float f = sm.tab[0 * 16 + tt] * wc - sm.tab[1 * 16 + tt] * wD * edv + sm.tab[2 * 16 + tt] * wR * g0;
     f *= rinv * keep;
     fx = fmaf(f, dx, fx);
@@ -94,33 +112,52 @@ __device__ __forceinline__ void pair_eval(const DevParams& P, const PairSmem& sm
   }
 }
 
-__device__ __forceinline__ PairSmem carve(unsigned char* base, int S, int NH, int NCB, int hcap, int lcap, int NT) {
-  PairSmem sm;
-  size_t o = 0;
-  sm.spos = (float4*)(base + o); o += (size_t)hcap * 16;
-  sm.svel = (float4*)(base + o); o += (size_t)hcap * 16;
-  sm.smeta = (uint32_t*)(base + o); o += (size_t)hcap * 4;
-  sm.scx = (float*)(base + o); o += (size_t)(S - 1) * hcap * 4;
-  sm.tab = (float*)(base + o); o += 8 * 16 * 4;
-  sm.hs = (int*)(base + o); o += (size_t)(NH + 1) * 4;
-  sm.bcs = (int*)(base + o); o += (size_t)(NCB + 1) * 4;
-  sm.bh = (int*)(base + o); o += (size_t)NCB * 4;
-  o = (o + 15) & ~(size_t)15;
-  sm.list = (uint16_t*)(base + o);
-  return sm;
+// evaluates `cnt` entries of one end of the list, two per iteration; entry k of the end lives at base + k * stride
+template <int S, bool RANDFLUX, bool FASTW, int MODE>
+__device__ __forceinline__ void eval_list(const DevParams& P, const PairArgs& A, const PairSmem& sm, const Self& me,
+                                          const uint16_t* base, int stride, int cnt, float& fx, float& fy, float& fz,
+                                          float* q) {
+  for (int k = 0; k < cnt; k += 2) {
+    const bool two = k + 1 < cnt;
+    const uint32_t e0 = base[k * stride];
+    const uint32_t e1 = two ? base[(k + 1) * stride] : e0;
+    pair_eval<S, RANDFLUX, FASTW, MODE>(P, A, sm, me, e0, 1.0f, fx, fy, fz, q);
+    pair_eval<S, RANDFLUX, FASTW, MODE>(P, A, sm, me, e1, two ? 1.0f : 0.0f, fx, fy, fz, q);
+  }
 }
 
-template <int S, bool RANDFLUX, bool FASTW>
-__global__ void __launch_bounds__(256) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
+// RING: 1 = r_cc >= r_c (ring entries are flux-only), 2 = r_c > r_cc (ring entries are force-only)
+template <int S, bool RANDFLUX, bool FASTW, int RING>
+__global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int NT = blockDim.x, t = threadIdx.x, lane = t & 31, warp = t >> 5, nwarp = NT >> 5;
-  const int HX = A.bx + 2, HY = A.by + 2, HZ = A.bz + 2, NH = HX * HY * HZ, NCB = A.bx * A.by * A.bz;
-  const int hcap = A.hcap, lcap = A.lcap;
-  PairSmem sm = carve(smem_raw, S, NH, NCB, hcap, lcap, NT);
-  __shared__ int s_src[6 * 6 * 6];     // first global slot of each halo cell
-  __shared__ float s_shift[6 * 6 * 6][3];
-  const Brick B = A.bricks[blockIdx.x];
+  const int NT = blockDim.x, t = threadIdx.x;
+  const int lcap = A.lcap;
+  PairSmem sm;
+  sm.tso = (float4*)smem_raw;
+  sm.tcnt = (uint32_t*)(smem_raw + (size_t)MAXLOC * 27 * 16);
+  sm.tab = (float*)(smem_raw + (size_t)MAXLOC * 27 * 20);
+  sm.list = (uint16_t*)(smem_raw + (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4);
 
+  const int64_t n = A.n;
+  const int64_t i0 = (int64_t)blockIdx.x * NT, i = i0 + t;
+  const bool active = i < n;
+  const int64_t ilast = (i0 + NT < n ? i0 + NT : n) - 1;
+  const uint32_t r_first = __ldg(&A.keys[i0]), r_last = __ldg(&A.keys[ilast]);
+  const uint32_t ri = active ? __ldg(&A.keys[i]) : 0xFFFFFFFFu;
+
+  Self me;
+  {
+    const int64_t is = active ? i : i0;
+    const float4 p = __ldg(&A.rec.P4[is]);
+    const float4 x = __ldg(&A.rec.X4[is]);
+    me.x = p.x; me.y = p.y; me.z = p.z;
+    me.id = __float_as_uint(p.w);
+    me.meta = __float_as_uint(x.z);
+    me.v = __ldg(&A.vel[is]);
+    me.c[0] = x.x; me.c[1] = x.y; me.c[2] = 0.f; me.c[3] = 0.f;
+    if (S > 2) { const float2 y = __ldg(&A.rec.Y2[is]); me.c[2] = y.x; me.c[3] = y.y; }
+    me.lc27 = 0;
+  }
   // ---- type-pair tables
   for (int k = t; k < 16; k += NT) {
     sm.tab[0 * 16 + k] = P.a[k];
@@ -130,185 +167,118 @@ __global__ void __launch_bounds__(256) k_pair(const __grid_constant__ DevParams 
 #pragma unroll
     for (int s = 0; s < TD_S; ++s) sm.tab[(4 + s) * 16 + k] = P.kappa[s][k];
   }
-  // ---- halo cells: counts, sources, image shifts
-  for (int h = t; h < NH; h += NT) {
-    int hx = h % HX, hy = (h / HX) % HY, hz = h / (HX * HY);
-    int c[3] = {B.ox + hx - 1, B.oy + hy - 1, B.oz + hz - 1};
-    int o[3] = {B.ox, B.oy, B.oz};
-    float sh[3];
-    bool exists = true;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-      int wimg = 0;
-      if (c[a] < 0) { c[a] += P.ncell[a]; wimg = -1; }
-      else if (c[a] >= P.ncell[a]) { c[a] -= P.ncell[a]; wimg = 1; }
-      // cells beyond a partial brick's extent that would wrap twice cannot occur: ncell >= 3, brick inside the grid
-      if (c[a] < 0 || c[a] >= P.ncell[a]) exists = false;
-      sh[a] = (float)o[a] * P.cell_edge[a] - (float)wimg * P.box[a];
-    }
-    uint32_t s0 = 0, s1 = 0;
-    if (exists) {
-      uint32_t rank = __ldg(&A.cell_rank[(c[2] * P.ncell[1] + c[1]) * P.ncell[0] + c[0]]);
-      s0 = __ldg(&A.cell_start[rank]);
-      s1 = __ldg(&A.cell_start[rank + 1]);
-    }
-    s_src[h] = (int)s0;
-    sm.hs[h + 1] = (int)(s1 - s0);
-    s_shift[h][0] = sh[0]; s_shift[h][1] = sh[1]; s_shift[h][2] = sh[2];
-  }
-  // ---- brick cells (Morton rank order): own-particle prefix and halo index
-  const uint32_t g0 = __ldg(&A.cell_start[B.r0]);
-  for (int c = t; c <= (int)B.ncell; c += NT) {
-    sm.bcs[c] = (int)(__ldg(&A.cell_start[B.r0 + c]) - g0);
-    if (c < (int)B.ncell) {
-      uint32_t pc = __ldg(&A.rank_cell[B.r0 + c]);
-      int cx = (int)(pc & 1023u) - B.ox, cy = (int)((pc >> 10) & 1023u) - B.oy, cz = (int)(pc >> 20) - B.oz;
-      sm.bh[c] = ((cz + 1) * HY + (cy + 1)) * HX + (cx + 1);
-    }
-  }
-  __syncthreads();
-  // ---- exclusive scan of halo counts (warp 0, chunks of 32 with carry)
-  if (warp == 0) {
-    int carry = 0;
-    if (lane == 0) sm.hs[0] = 0;
-    for (int b0 = 0; b0 < NH; b0 += 32) {
-      int h = b0 + lane;
-      int v = h < NH ? sm.hs[h + 1] : 0, x = v;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        int y = __shfl_up_sync(0xffffffffu, x, d);
-        if (lane >= d) x += y;
-      }
-      if (h < NH) sm.hs[h + 1] = carry + x;
-      carry += __shfl_sync(0xffffffffu, x, 31);
-    }
-  }
-  __syncthreads();
-  const int nh = sm.hs[NH];
-  const int nb = sm.bcs[B.ncell];  // particles owned by this brick
-  if (nh > hcap) {                 // cannot stage: report, never write out of bounds
-    if (t == 0) atomicOr(A.err, TD_ERR_HALO_OVERFLOW);
-    return;
-  }
-  // ---- stage the halo: one warp per halo cell, coordinates relative to the brick origin
-  const int64_t n = A.n;
-  for (int h = warp; h < NH; h += nwarp) {
-    int d0 = sm.hs[h], cnt = sm.hs[h + 1] - d0, s0 = s_src[h];
-    float sx = s_shift[h][0], sy = s_shift[h][1], sz = s_shift[h][2];
-    for (int k = lane; k < cnt; k += 32) {
-      float4 p = A.st.pos[s0 + k];
-      float4 l = A.st.lo[s0 + k];
-      p.x = (p.x - sx) + l.x; p.y = (p.y - sy) + l.y; p.z = (p.z - sz) + l.z;
-      sm.spos[d0 + k] = p;
-      sm.svel[d0 + k] = A.st.vel[s0 + k];
-      sm.smeta[d0 + k] = __float_as_uint(l.w);
-#pragma unroll
-      for (int s = 1; s < S; ++s) sm.scx[(s - 1) * hcap + d0 + k] = A.st.cx[(int64_t)(s - 1) * n + s0 + k];
-    }
-  }
-  __syncthreads();
+  const float rin2 = fminf(P.rc2, P.rcc2), rout2 = P.rcut2;
+  uint16_t* const lfront = sm.list + t;
+  uint16_t* const lback = sm.list + (size_t)(lcap - 1) * NT + t;
 
-  // ---- particles of the brick, NT at a time (normally one round)
-  for (int p0 = 0; p0 < nb; p0 += NT) {
-    const int ip = p0 + t;
-    const bool active = ip < nb;
-    int self = 0, cbx = 0, cby = 0, cbz = 0;
-    if (active) {
-      int lo = 0, hi = (int)B.ncell;  // find brick cell c with bcs[c] <= ip < bcs[c+1]
-      while (hi - lo > 1) {
-        int mid = (lo + hi) >> 1;
-        if (sm.bcs[mid] <= ip) lo = mid; else hi = mid;
-      }
-      int hcell = sm.bh[lo];
-      self = sm.hs[hcell] + (ip - sm.bcs[lo]);
-      cbx = hcell % HX - 1; cby = (hcell / HX) % HY - 1; cbz = hcell / (HX * HY) - 1;
-    }
-    float4 pi = sm.spos[active ? self : 0];
-    float4 vi = sm.svel[active ? self : 0];
-    uint32_t mi = sm.smeta[active ? self : 0];
-    uint32_t idi = __float_as_uint(pi.w);
-    float ci[S];
-    ci[0] = vi.w;
+  for (uint32_t rb = r_first; rb <= r_last; rb += MAXLOC) {
+    const int nloc = (int)min((uint32_t)MAXLOC, r_last - rb + 1u);
+    __syncthreads();
+    // ---- neighbour table of the cells rb .. rb + nloc - 1
+    for (int idx = t; idx < nloc * 27; idx += NT) {
+      const int lc = idx / 27, c = idx - lc * 27;
+      const uint32_t pc = __ldg(&A.rank_cell[rb + lc]);
+      const int d[3] = {c % 3 - 1, (c / 3) % 3 - 1, c / 9 - 1};
+      int cc[3] = {(int)(pc & 1023u) + d[0], (int)((pc >> 10) & 1023u) + d[1], (int)(pc >> 20) + d[2]};
+      float off[3];
 #pragma unroll
-    for (int s = 1; s < S; ++s) ci[s] = sm.scx[(s - 1) * hcap + (active ? self : 0)];
+      for (int a = 0; a < 3; ++a) {
+        float w = 0.0f;
+        if (cc[a] < 0) { cc[a] += P.ncell[a]; w = -1.0f; }
+        else if (cc[a] >= P.ncell[a]) { cc[a] -= P.ncell[a]; w = 1.0f; }
+        off[a] = fmaf(w, P.gap[a], (float)d[a] * P.edge_q[a]);  // origin of the neighbour image - own origin
+      }
+      const uint32_t rk = __ldg(&A.cell_rank[(cc[2] * P.ncell[1] + cc[1]) * P.ncell[0] + cc[0]]);
+      const uint32_t s0 = __ldg(&A.cell_start[rk]), s1 = __ldg(&A.cell_start[rk + 1]);
+      uint32_t cnt = s1 - s0;
+      if (cnt > OFFMASK) { cnt = OFFMASK; atomicOr(A.err, TD_ERR_CELL_OVERFLOW); }
+      sm.tso[idx] = make_float4(__uint_as_float(s0), off[0], off[1], off[2]);
+      sm.tcnt[idx] = cnt;
+    }
+    __syncthreads();
+    const bool mine = active && ri >= rb && ri - rb < (uint32_t)nloc;
+    me.lc27 = mine ? (int)(ri - rb) * 27 : 0;
+
     float fx = 0.f, fy = 0.f, fz = 0.f, q[S];
 #pragma unroll
     for (int s = 0; s < S; ++s) q[s] = 0.f;
     int nA = 0, nB = 0;
 
     auto flush = [&]() {
-      for (int k = 0; k < nA; ++k)
-        pair_eval<S, RANDFLUX, FASTW, true>(P, sm, hcap, sm.list[k * NT + t], pi.x, pi.y, pi.z, vi, ci, idi, mi, A.step,
-                                            fx, fy, fz, q);
-      for (int k = 0; k < nB; ++k)
-        pair_eval<S, RANDFLUX, FASTW, false>(P, sm, hcap, sm.list[(lcap - 1 - k) * NT + t], pi.x, pi.y, pi.z, vi, ci,
-                                             idi, mi, A.step, fx, fy, fz, q);
+      eval_list<S, RANDFLUX, FASTW, 0>(P, A, sm, me, lfront, NT, nA, fx, fy, fz, q);
+      eval_list<S, RANDFLUX, FASTW, RING>(P, A, sm, me, lback, -NT, nB, fx, fy, fz, q);
       nA = 0; nB = 0;
     };
 
-    for (int run = 0; run < 9; ++run) {
-      int k = 0, kend = 0;
-      if (active) {
-        int hrow = ((cbz + run / 3) * HY + (cby + run % 3)) * HX + cbx;  // halo cell (cbx-1+1, ...) = first of the run
-        k = sm.hs[hrow];
-        kend = sm.hs[hrow + 3];
-      }
+    for (int c = 0; c < 27; ++c) {
+      const float4 te = sm.tso[me.lc27 + c];
+      const int cnt = mine ? (int)sm.tcnt[me.lc27 + c] : 0;
+      const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x);
+      const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
+      const uint32_t ebase = (uint32_t)c << OFFBITS;
+      int k = 0;
       while (true) {
-        int ke = min(kend, k + (lcap - nA - nB));
-        for (; k < ke; ++k) {
-          float4 pj = sm.spos[k];
-          float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-          float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-          if (r2 < P.rcut2 && r2 >= 1e-12f) {  // R22: coincident particles (and self) skipped
-            if (r2 < P.rc2) { sm.list[nA * NT + t] = (uint16_t)k; ++nA; }
-            else if (r2 < P.rcc2) { sm.list[(lcap - 1 - nB) * NT + t] = (uint16_t)k; ++nB; }
-          }
+        const int kend = min(cnt, k + (lcap - nA - nB));
+        uint16_t* pa = lfront + nA * NT;
+        uint16_t* pb = lback - nB * NT;
+#pragma unroll 4
+        for (; k < kend; ++k) {
+          const float4 pj = __ldg(&src[k]);
+          const float dx = xs - pj.x, dy = ys - pj.y, dz = zs - pj.z;
+          const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+          const bool in = r2 < rin2;
+          const bool ring = !in && r2 < rout2;
+          const uint16_t ent = (uint16_t)(ebase | (uint32_t)k);
+          if (in) { *pa = ent; pa += NT; ++nA; }
+          if (ring) { *pb = ent; pb -= NT; ++nB; }
         }
-        if (!__any_sync(0xffffffffu, k < kend)) break;
+        if (!__any_sync(0xffffffffu, k < cnt)) break;
         flush();  // some lane's list is full
       }
     }
     flush();
-    if (active) {
-      int64_t slot = (int64_t)g0 + ip;
-      A.F4[slot] = make_float4(fx, fy, fz, q[0]);
+    if (mine) {
+      A.F4[i] = make_float4(fx, fy, fz, q[0]);
 #pragma unroll
-      for (int s = 1; s < S; ++s) A.Qx[(int64_t)(s - 1) * n + slot] = q[s];
+      for (int s = 1; s < S; ++s) A.Qx[(int64_t)(s - 1) * n + i] = q[s];
     }
   }
 }
 
 template <int S>
-int launch_s(const DevParams& P, const PairArgs& A, int nbricks, int nthreads, size_t smem, cudaStream_t st) {
-#define TD_PAIR_GO(RF, FW)                                                                                   \
+int launch_s(const DevParams& P, const PairArgs& A, int nblk, int nthreads, size_t smem, cudaStream_t st) {
+#define TD_PAIR_GO(RF, FW, RG)                                                                               \
   do {                                                                                                       \
-    auto kf = k_pair<S, RF, FW>;                                                                             \
+    auto kf = k_pair<S, RF, FW, RG>;                                                                         \
     cudaError_t e = cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);       \
     if (e != cudaSuccess) return (int)e;                                                                     \
-    kf<<<nbricks, nthreads, smem, st>>>(P, A);                                                               \
+    kf<<<nblk, nthreads, smem, st>>>(P, A);                                                                  \
   } while (0)
-  if (P.rand_flux) { if (P.fast_w) TD_PAIR_GO(true, true); else TD_PAIR_GO(true, false); }
-  else { if (P.fast_w) TD_PAIR_GO(false, true); else TD_PAIR_GO(false, false); }
+  const bool ring1 = P.rcc2 >= P.rc2;
+  if (P.rand_flux) {
+    if (P.fast_w) { if (ring1) TD_PAIR_GO(true, true, 1); else TD_PAIR_GO(true, true, 2); }
+    else { if (ring1) TD_PAIR_GO(true, false, 1); else TD_PAIR_GO(true, false, 2); }
+  } else {
+    if (P.fast_w) { if (ring1) TD_PAIR_GO(false, true, 1); else TD_PAIR_GO(false, true, 2); }
+    else { if (ring1) TD_PAIR_GO(false, false, 1); else TD_PAIR_GO(false, false, 2); }
+  }
 #undef TD_PAIR_GO
   return 0;
 }
 }  // namespace
 
-size_t td_pair_smem_bytes(int S, int bx, int by, int bz, int hcap, int lcap, int nthreads) {
-  int NH = (bx + 2) * (by + 2) * (bz + 2), NCB = bx * by * bz;
-  size_t o = (size_t)hcap * (16 + 16 + 4 + 4 * (S - 1)) + 8 * 16 * 4 + (size_t)(NH + 1) * 4 + (size_t)(NCB + 1) * 4 +
-             (size_t)NCB * 4;
-  o = (o + 15) & ~(size_t)15;
-  return o + (size_t)lcap * nthreads * 2;
+size_t td_pair_smem_bytes(int lcap, int nthreads) {
+  return (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4 + (size_t)lcap * nthreads * 2;
 }
 
-int td_launch_pair(const DevParams& P, const PairArgs& A, int nbricks, int nthreads, cudaStream_t st) {
-  if (nbricks == 0) return 0;
-  size_t smem = td_pair_smem_bytes(P.n_species, A.bx, A.by, A.bz, A.hcap, A.lcap, nthreads);
+int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st) {
+  if (A.n == 0) return 0;
+  const size_t smem = td_pair_smem_bytes(A.lcap, nthreads);
+  const int nblk = (int)((A.n + nthreads - 1) / nthreads);
   switch (P.n_species) {
-    case 1: return launch_s<1>(P, A, nbricks, nthreads, smem, st);
-    case 2: return launch_s<2>(P, A, nbricks, nthreads, smem, st);
-    case 3: return launch_s<3>(P, A, nbricks, nthreads, smem, st);
-    default: return launch_s<4>(P, A, nbricks, nthreads, smem, st);
+    case 1: return launch_s<1>(P, A, nblk, nthreads, smem, st);
+    case 2: return launch_s<2>(P, A, nblk, nthreads, smem, st);
+    case 3: return launch_s<3>(P, A, nblk, nthreads, smem, st);
+    default: return launch_s<4>(P, A, nblk, nthreads, smem, st);
   }
 }

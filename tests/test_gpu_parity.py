@@ -107,13 +107,14 @@ def test_config1_one_step_forces(T, orc):
     check_forces(sim, o, label="config1 step 3")
 
 
-@pytest.mark.parametrize("brick", [3, 4, 5])
-def test_brick_shapes_agree(T, orc, brick):
-    w = W.make_fluid("t", (13, 11, 8), 4.0, seed=21)  # 8 x 6 x 5 cells: partial bricks on every axis
-    sim = T.Simulation.from_workload(w, brick_log2=brick)
+@pytest.mark.parametrize("nt,cap", [(32, 4), (64, 16), (128, 0), (256, 0), (256, 7)])
+def test_pair_launch_shapes_agree(T, orc, nt, cap):
+    # 8 x 6 x 5 cells (not powers of two: holes in the Morton rank range); tiny list caps force mid-scan flushes
+    w = W.make_fluid("t", (13, 11, 8), 4.0, seed=21)
+    sim = T.Simulation.from_workload(w, pair_threads=nt, list_cap=cap)
     o = orc.Oracle.from_workload(w)
     o.compute_forces(0)
-    check_forces(sim, o, label=f"brick {brick}")
+    check_forces(sim, o, label=f"pair_threads {nt} list_cap {cap}")
 
 
 def test_random_flux_off_and_general_exponents(T, orc):
