@@ -387,7 +387,7 @@ static void build_grid(tdpd_sim* s) {
   {
     double rcut = std::max(s->prm.r_c, s->prm.r_cc);
     double mn = 4.18879 * rcut * rcut * rcut * (double)s->n / ((double)s->prm.box[0] * s->prm.box[1] * s->prm.box[2]);
-    int lc = ((int)(mn * 1.2) + 6 + 1) / 2 * 2;
+    int lc = ((int)(mn * 1.4) + 8 + 1) / 2 * 2;
     s->lcap = s->tune_lcap ? s->tune_lcap : std::min(160, std::max(16, lc));
     int nt = s->n >= 148 * 8 * 256 ? 256 : (s->n >= 148 * 8 * 128 ? 128 : 64);
     s->pair_nt = s->tune_nt ? s->tune_nt : nt;

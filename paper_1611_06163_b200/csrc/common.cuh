@@ -74,22 +74,38 @@ __device__ __forceinline__ float td_rsqrt_approx(float x) {
   return y;
 }
 
+__device__ __forceinline__ float td_lg2_approx(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float td_sin_approx(float x) {
+  float y;
+  asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float td_cos_approx(float x) {
+  float y;
+  asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 // Box-Muller: R = sqrt(-2 ln ua); (g_cos, g_sin) = R (cos 2 pi ub, sin 2 pi ub).
-// MUFU lg2/sin/cos; lg2.approx has absolute error 2^-22 on (0.5, 2), which is not good enough for R when
-// ua -> 1 (R -> 0), so the top 2^-17 of the range uses the series -2 ln(1 - t) = 2t + t^2 + O(t^3).
+// MUFU lg2/sqrt/sin/cos; lg2.approx has absolute error 2^-22 on (0.5, 2), which is not good enough for R when
+// ua -> 1 (R -> 0), so the top 2^-17 of the range uses the series -2 ln(1 - t) = 2t + t^2 + O(t^3) with
+// t = 1 - ua (exact in fp32).  Branch-free.
+__device__ __forceinline__ float td_bm_radius(uint32_t xa) {
+  const float u = td_uniform(xa);
+  const float t = 1.0f - u;
+  const float q1 = -1.3862943611198906f * td_lg2_approx(u);  // -2 ln 2 * lg2(u)
+  const float q2 = fmaf(t, t, t + t);
+  return td_sqrt_approx(t < 7.62939453125e-06f ? q2 : q1);
+}
 __device__ __forceinline__ void td_box_muller(uint32_t xa, uint32_t xb, float& g_cos, float& g_sin) {
-  float q;
-  if (xa >= 0xFFFF8000u) {
-    // t = 1 - ua = ((2^23 - 1 - (xa >> 9)) + 1/2) 2^-23, exact
-    float t = fmaf((float)(8388607u - (xa >> 9)), 1.1920928955078125e-07f, 5.9604644775390625e-08f);  // rare
-    q = fmaf(t, t, 2.0f * t);
-  } else {
-    q = -1.3862943611198906f * __log2f(td_uniform(xa));  // -2 ln 2 * lg2(u)
-  }
-  float R = td_sqrt_approx(q);
-  float ang = 6.283185307179586f * td_uniform(xb);
-  g_cos = R * __cosf(ang);
-  g_sin = R * __sinf(ang);
+  const float R = td_bm_radius(xa);
+  const float ang = 6.283185307179586f * td_uniform(xb);
+  g_cos = R * td_cos_approx(ang);
+  g_sin = R * td_sin_approx(ang);
 }
 
 // ---- kernel argument blocks -----------------------------------------------------------------------------

@@ -34,7 +34,7 @@ struct PairSmem {
 
 __device__ __forceinline__ float td_pow_w(float w, float s) {
   // w in (0,1], s >= 0
-  return s == 0.0f ? 1.0f : exp2f(s * __log2f(fmaxf(w, 0.0f)));
+  return s == 0.0f ? 1.0f : exp2f(s * td_lg2_approx(fmaxf(w, 1e-30f)));
 }
 
 struct Self {  // the thread's own particle
@@ -202,38 +202,50 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
     float fx = 0.f, fy = 0.f, fz = 0.f, q[S];
 #pragma unroll
     for (int s = 0; s < S; ++s) q[s] = 0.f;
-    int nA = 0, nB = 0;
+    // two-ended list: pa grows up from the front, pb down from the back (32-bit shared-memory addresses)
+    const uint32_t stride = 2u * (uint32_t)NT;
+    const int sh = 31 - __clz((int)stride);
+    const uint32_t lf32 = (uint32_t)__cvta_generic_to_shared(lfront), lb32 = (uint32_t)__cvta_generic_to_shared(lback);
+    uint32_t pa = lf32, pb = lb32;
 
     auto flush = [&]() {
-      eval_list<S, RANDFLUX, FASTW, 0>(P, A, sm, me, lfront, NT, nA, fx, fy, fz, q);
-      eval_list<S, RANDFLUX, FASTW, RING>(P, A, sm, me, lback, -NT, nB, fx, fy, fz, q);
-      nA = 0; nB = 0;
+      eval_list<S, RANDFLUX, FASTW, 0>(P, A, sm, me, lfront, NT, (int)((pa - lf32) >> sh), fx, fy, fz, q);
+      eval_list<S, RANDFLUX, FASTW, RING>(P, A, sm, me, lback, -NT, (int)((lb32 - pb) >> sh), fx, fy, fz, q);
+      pa = lf32; pb = lb32;
     };
 
     for (int c = 0; c < 27; ++c) {
       const float4 te = sm.tso[me.lc27 + c];
       const int cnt = mine ? (int)sm.tcnt[me.lc27 + c] : 0;
-      const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x);
-      const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
       const uint32_t ebase = (uint32_t)c << OFFBITS;
-      int k = 0;
+      const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x) - ebase;  // indexed by the list entry
+      const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
+      uint32_t e = ebase;
+      const uint32_t ecnt = ebase + (uint32_t)cnt;
       while (true) {
-        const int kend = min(cnt, k + (lcap - nA - nB));
-        uint16_t* pa = lfront + nA * NT;
-        uint16_t* pb = lback - nB * NT;
+        const uint32_t room = (uint32_t)(((int)(pb - pa) >> sh) + 1);  // free entries (pa <= pb + stride always)
+        const uint32_t eend = min(ecnt, e + room);
 #pragma unroll 4
-        for (; k < kend; ++k) {
-          const float4 pj = __ldg(&src[k]);
+        for (; e < eend; ++e) {
+          const float4 pj = __ldg(&src[e]);
           const float dx = xs - pj.x, dy = ys - pj.y, dz = zs - pj.z;
           const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-          const bool in = r2 < rin2;
-          const bool ring = !in && r2 < rout2;
-          const uint16_t ent = (uint16_t)(ebase | (uint32_t)k);
-          if (in) { *pa = ent; pa += NT; ++nA; }
-          if (ring) { *pb = ent; pb -= NT; ++nB; }
+          // branch-free push: front if r2 < rin2, back if rin2 <= r2 < rout2
+          asm volatile(
+              "{\n\t.reg .pred pin, prg;\n\t"
+              "setp.lt.f32 pin, %2, %3;\n\t"
+              "setp.lt.and.f32 prg, %2, %4, !pin;\n\t"
+              "@pin st.shared.u16 [%0], %5;\n\t"
+              "@prg st.shared.u16 [%1], %5;\n\t"
+              "@pin add.u32 %0, %0, %6;\n\t"
+              "@prg sub.u32 %1, %1, %6;\n\t}"
+              : "+r"(pa), "+r"(pb)
+              : "f"(r2), "f"(rin2), "f"(rout2), "h"((uint16_t)e), "r"(stride)
+              : "memory");
         }
-        if (!__any_sync(0xffffffffu, k < cnt)) break;
-        flush();  // some lane's list is full
+        const bool more = e < ecnt;
+        if (!__any_sync(0xffffffffu, more)) break;
+        if (__any_sync(0xffffffffu, more && pa > pb)) flush();  // some lane's list is full
       }
     }
     flush();
