@@ -202,27 +202,22 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
     float fx = 0.f, fy = 0.f, fz = 0.f, q[S];
 #pragma unroll
     for (int s = 0; s < S; ++s) q[s] = 0.f;
-    // two-ended list: pa grows up from the front, pb down from the back (32-bit shared-memory addresses)
+    // two-ended stack: pa grows up from the front, pb down from the back (32-bit shared-memory addresses).
+    // Entries are evaluated in warp-uniform batches popped from the tops: after every scanned cell the warp takes
+    // the largest multiple of BA (BB) entries that EVERY lane owns, so all lanes run the expensive loops together;
+    // a lane whose stack is full, or the end of the stencil, drains everything.
+    constexpr int BA = 4, BB = 8;
     const uint32_t stride = 2u * (uint32_t)NT;
     const int sh = 31 - __clz((int)stride);
     const uint32_t lf32 = (uint32_t)__cvta_generic_to_shared(lfront), lb32 = (uint32_t)__cvta_generic_to_shared(lback);
     uint32_t pa = lf32, pb = lb32;
-
-    auto flush = [&]() {
-      eval_list<S, RANDFLUX, FASTW, 0>(P, A, sm, me, lfront, NT, (int)((pa - lf32) >> sh), fx, fy, fz, q);
-      eval_list<S, RANDFLUX, FASTW, RING>(P, A, sm, me, lback, -NT, (int)((lb32 - pb) >> sh), fx, fy, fz, q);
-      pa = lf32; pb = lb32;
-    };
-
-    for (int c = 0; c < 27; ++c) {
-      const float4 te = sm.tso[me.lc27 + c];
-      const int cnt = mine ? (int)sm.tcnt[me.lc27 + c] : 0;
-      const uint32_t ebase = (uint32_t)c << OFFBITS;
-      const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x) - ebase;  // indexed by the list entry
-      const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
-      uint32_t e = ebase;
-      const uint32_t ecnt = ebase + (uint32_t)cnt;
-      while (true) {
+    int c = 0;
+    float4 te = sm.tso[me.lc27];
+    uint32_t e = 0, ecnt = mine ? sm.tcnt[me.lc27] : 0u;
+    while (true) {
+      {
+        const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x) - ((uint32_t)c << OFFBITS);  // by entry
+        const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
         const uint32_t room = (uint32_t)(((int)(pb - pa) >> sh) + 1);  // free entries (pa <= pb + stride always)
         const uint32_t eend = min(ecnt, e + room);
 #pragma unroll 4
@@ -243,12 +238,33 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
               : "f"(r2), "f"(rin2), "f"(rout2), "h"((uint16_t)e), "r"(stride)
               : "memory");
         }
-        const bool more = e < ecnt;
-        if (!__any_sync(0xffffffffu, more)) break;
-        if (__any_sync(0xffffffffu, more && pa > pb)) flush();  // some lane's list is full
+      }
+      const bool more = e < ecnt;
+      const bool anymore = __any_sync(0xffffffffu, more);
+      const int nA = (int)((pa - lf32) >> sh), nB = (int)((lb32 - pb) >> sh);
+      int dA, dB;
+      if ((!anymore && c == 26) || __any_sync(0xffffffffu, more && pa > pb)) {
+        dA = nA; dB = nB;
+      } else {
+        const int mA = __reduce_min_sync(0xffffffffu, mine ? nA : 0x7fffffff);
+        const int mB = __reduce_min_sync(0xffffffffu, mine ? nB : 0x7fffffff);
+        dA = mine ? (mA & ~(BA - 1)) : 0;
+        dB = mine ? (mB & ~(BB - 1)) : 0;
+      }
+      if (__any_sync(0xffffffffu, (dA | dB) != 0)) {
+        eval_list<S, RANDFLUX, FASTW, 0>(P, A, sm, me, lfront + (nA - dA) * NT, NT, dA, fx, fy, fz, q);
+        eval_list<S, RANDFLUX, FASTW, RING>(P, A, sm, me, lback - (nB - dB) * NT, -NT, dB, fx, fy, fz, q);
+        pa -= (uint32_t)dA * stride;
+        pb += (uint32_t)dB * stride;
+      }
+      if (!anymore) {
+        if (c == 26) break;
+        ++c;
+        te = sm.tso[me.lc27 + c];
+        e = (uint32_t)c << OFFBITS;
+        ecnt = e + (mine ? sm.tcnt[me.lc27 + c] : 0u);
       }
     }
-    flush();
     if (mine) {
       A.F4[i] = make_float4(fx, fy, fz, q[0]);
 #pragma unroll
