@@ -54,6 +54,7 @@ struct tdpd_sim {
   uint32_t ncells = 0;
   int key_bits = 0;
   std::vector<uint32_t> cell_rank, rank_cell;
+  std::vector<uint32_t> seg_off, seg_first, seg_meta;  // static neighbour runs of every cell (PairArgs)
   int pair_nt = 256, lcap = 72, tune_nt = 0, tune_lcap = 0;
   PairRec rec = {nullptr, nullptr, nullptr};
   uint32_t* keys_sorted = nullptr;
@@ -67,6 +68,7 @@ struct tdpd_sim {
   uint32_t *keys[2] = {nullptr, nullptr}, *vals[2] = {nullptr, nullptr};
   void* sort_scratch = nullptr;
   uint32_t *cell_start = nullptr, *cell_rank_d = nullptr, *rank_cell_d = nullptr, *slot_of_id = nullptr;
+  uint32_t *seg_off_d = nullptr, *seg_first_d = nullptr, *seg_meta_d = nullptr;
   float4 *F4 = nullptr, *Fb = nullptr;
   float *Qx = nullptr, *staging = nullptr;
   int* err_d = nullptr;
@@ -382,6 +384,50 @@ static void build_grid(tdpd_sim* s) {
     uint32_t x = lin % nc[0], y = (lin / nc[0]) % nc[1], z = lin / (nc[0] * nc[1]);
     s->rank_cell[r] = x | (y << 10) | (z << 20);
   }
+  // static neighbour runs: the 27 neighbours of a cell, sorted by Morton rank, merged while they are
+  // rank-consecutive and share the 2x2x2 block and the periodic image (one displacement per run)
+  if (s->seg_off.size() != (size_t)s->ncells + 1) {
+    s->seg_off.assign((size_t)s->ncells + 1, 0);
+    s->seg_first.clear(); s->seg_meta.clear();
+    s->seg_first.reserve((size_t)s->ncells * 14); s->seg_meta.reserve((size_t)s->ncells * 14);
+    for (uint32_t r = 0; r < s->ncells; ++r) {
+      const uint32_t pc = s->rank_cell[r];
+      const int c[3] = {(int)(pc & 1023u), (int)((pc >> 10) & 1023u), (int)(pc >> 20)};
+      std::pair<uint32_t, uint64_t> nb[27];  // (rank, signature = block | wrap code << 27)
+      for (int k = 0; k < 27; ++k) {
+        const int d[3] = {k % 3 - 1, (k / 3) % 3 - 1, k / 9 - 1};
+        int q[3];
+        uint32_t wcode = 0;
+        for (int a = 0; a < 3; ++a) {
+          q[a] = c[a] + d[a];
+          int w = 0;
+          if (q[a] < 0) { q[a] += nc[a]; w = -1; }
+          else if (q[a] >= nc[a]) { q[a] -= nc[a]; w = 1; }
+          wcode |= (uint32_t)(w + 1) << (2 * a);
+        }
+        const uint32_t rank = s->cell_rank[(size_t)(q[2] * nc[1] + q[1]) * nc[0] + q[0]];
+        const uint32_t blk = (uint32_t)(q[0] >> 1) | ((uint32_t)(q[1] >> 1) << 9) | ((uint32_t)(q[2] >> 1) << 18);
+        nb[k] = {rank, (uint64_t)blk | ((uint64_t)wcode << 27)};
+      }
+      std::sort(nb, nb + 27);
+      std::pair<int, std::pair<uint32_t, uint32_t>> runs[27];  // (-cells, (first rank, meta))
+      int nr = 0;
+      for (int k = 0; k < 27;) {
+        int m = 1;
+        while (k + m < 27 && m < 15 && nb[k + m].first == nb[k].first + (uint32_t)m && nb[k + m].second == nb[k].second) ++m;
+        runs[nr++] = {-m, {nb[k].first, (uint32_t)m | ((uint32_t)(nb[k].second >> 27) << 4)}};
+        k += m;
+      }
+      // longest runs first: every interior cell has the same multiset of run sizes (8, 4, 2, 2, 2, 1 x 9), so the
+      // k-th run of all lanes of a warp has the same number of cells and the scan loops stay in step
+      std::sort(runs, runs + nr);
+      for (int k = 0; k < nr; ++k) {
+        s->seg_first.push_back(runs[k].second.first);
+        s->seg_meta.push_back(runs[k].second.second);
+      }
+      s->seg_off[r + 1] = (uint32_t)s->seg_first.size();
+    }
+  }
   // launch configuration of the pair kernel: NT consecutive slots per CTA; small systems use smaller CTAs so that
   // every SM gets several; the two-ended hit list holds ~1.3 x the mean number of neighbours inside the cutoff
   {
@@ -430,6 +476,9 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->cell_start = c.take<uint32_t>(s->ncells + 1);
   s->cell_rank_d = c.take<uint32_t>(s->ncells);
   s->rank_cell_d = c.take<uint32_t>(s->ncells);
+  s->seg_off_d = c.take<uint32_t>(s->seg_off.size());
+  s->seg_first_d = c.take<uint32_t>(s->seg_first.size());
+  s->seg_meta_d = c.take<uint32_t>(s->seg_meta.size());
   s->rec.P4 = c.take<float4>(n);
   s->rec.X4 = c.take<float4>(n);
   s->rec.Y2 = c.take<float2>(S > 2 ? n : 1);
@@ -510,6 +559,9 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
   }
   CK(cudaMemcpyAsync(s->cell_rank_d, s->cell_rank.data(), s->ncells * 4, cudaMemcpyHostToDevice, q));
   CK(cudaMemcpyAsync(s->rank_cell_d, s->rank_cell.data(), s->ncells * 4, cudaMemcpyHostToDevice, q));
+  CK(cudaMemcpyAsync(s->seg_off_d, s->seg_off.data(), s->seg_off.size() * 4, cudaMemcpyHostToDevice, q));
+  CK(cudaMemcpyAsync(s->seg_first_d, s->seg_first.data(), s->seg_first.size() * 4, cudaMemcpyHostToDevice, q));
+  CK(cudaMemcpyAsync(s->seg_meta_d, s->seg_meta.data(), s->seg_meta.size() * 4, cudaMemcpyHostToDevice, q));
   // membranes
   std::vector<MeshTemplateDev> td(s->tmpls.size());
   std::vector<unsigned char> topo;
@@ -622,6 +674,7 @@ int eval_forces(tdpd_sim* s) {
     PairArgs A;
     A.rec = s->rec; A.vel = s->st[c].vel; A.keys = s->keys_sorted;
     A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
+    A.seg_off = s->seg_off_d; A.seg_first = s->seg_first_d; A.seg_meta = s->seg_meta_d;
     A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step = (uint32_t)s->step; A.lcap = s->lcap; A.err = s->err_d;
     int rc = td_launch_pair(s->dp, A, s->pair_nt, s->sA);
     if (rc) return fail(s, TDPD_ECUDA, std::string("pair kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));

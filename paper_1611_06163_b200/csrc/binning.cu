@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
 }
 
 // gather the state into the new order, record slot_of_id for membrane vertices, fill the cell-start table and
-// write the pair kernel's records: position relative to the cell origin o_c = c * edge_q (exact product; the
+// write the pair kernel's records: position relative to the block origin (c & ~1) * edge_q (exact product; the
 // subtraction hi - o_c is exact too, so rel carries the full two-float position to ~2^-24), id, concentrations, meta
 template <int S>
 __global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState src, SortedState dst, PairRec rec,
@@ -147,8 +147,8 @@ __global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState 
     dst.cx[(int64_t)(s - 1) * n + i] = cxv[s - 1];
   }
   const uint32_t pc = __ldg(&rank_cell[k]);
-  const float ox = (float)(pc & 1023u) * P.edge_q[0], oy = (float)((pc >> 10) & 1023u) * P.edge_q[1],
-              oz = (float)(pc >> 20) * P.edge_q[2];
+  const float ox = (float)(pc & 1022u) * P.edge_q[0], oy = (float)((pc >> 10) & 1022u) * P.edge_q[1],
+              oz = (float)((pc >> 20) & 1022u) * P.edge_q[2];  // origin of the 2x2x2 block
   rec.P4[i] = make_float4(__fadd_rn(__fsub_rn(p.x, ox), l.x), __fadd_rn(__fsub_rn(p.y, oy), l.y),
                           __fadd_rn(__fsub_rn(p.z, oz), l.z), p.w);
   rec.X4[i] = make_float4(v.w, cxv[0], l.w, 0.0f);

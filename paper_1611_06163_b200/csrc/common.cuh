@@ -15,9 +15,9 @@ struct DevParams {
   int ncell[3];
   float cell_inv[3];   // (float)(n_a / L_a): binning multiplier (R-bin)
   float cell_edge[3];  // L_a / n_a
-  // pair-kernel coordinates are stored RELATIVE to a per-cell origin o_c = c * edge_q (exact in fp32: edge_q keeps
-  // 13 significant bits and c < 1024), so that differences between neighbouring cells are exact; gap = L - n edge_q
-  // is the extra displacement across the periodic boundary
+  // pair-kernel coordinates are stored RELATIVE to the origin of the particle's 2x2x2 cell block,
+  // o = (c & ~1) * edge_q (exact in fp32: edge_q keeps 13 significant bits and c < 1024), so that differences
+  // between neighbouring blocks are exact; gap = L - n edge_q (kept for reference)
   float edge_q[3], gap[3];
   float r_c, r_cc, rc2, rcc2, rcut2, inv_rc, inv_rcc;
   float dt, half_dt;
@@ -118,7 +118,7 @@ struct SortedState {   // one side of the ping-pong, cell-sorted order
 
 // pair-kernel records, written by the reorder kernel in cell-sorted order (read-only in the pair kernel)
 struct PairRec {
-  float4* P4;   // x, y, z relative to the cell origin o_c (see DevParams::edge_q), id (bits)
+  float4* P4;   // x, y, z relative to the origin of the 2x2x2 cell block, (c & ~1) * edge_q (see DevParams), id (bits)
   float4* X4;   // C_0, C_1, td_meta (bits), 0
   float2* Y2;   // C_2, C_3 (only when n_species > 2)
 };
@@ -129,7 +129,12 @@ struct PairArgs {
   const uint32_t* keys;        // [n] Morton rank of the cell of each slot (sorted)
   const uint32_t* cell_start;  // [ncell + 1] by Morton rank
   const uint32_t* cell_rank;   // [ncell] x-fastest linear cell -> Morton rank
-  const uint32_t* rank_cell;   // [ncell] Morton rank -> packed cx | cy << 10 | cz << 20
+ const uint32_t* rank_cell;   // [ncell] Morton rank -> packed cx | cy << 10 | cz << 20
+  // static neighbour segments of every cell (CSR by Morton rank): runs of rank-consecutive neighbour cells that
+  // lie in one 2x2x2 block and one periodic image, so that one displacement serves the whole run
+  const uint32_t* seg_off;     // [ncell + 1]
+  const uint32_t* seg_first;   // first Morton rank of the run
+  const uint32_t* seg_meta;    // cells in the run | (wrap_x + 1) << 4 | (wrap_y + 1) << 6 | (wrap_z + 1) << 8
   float4* F4;                  // Fx, Fy, Fz, Q_0 by slot
   float* Qx;                   // [(S-1)][n]
   int64_t n;

@@ -26,8 +26,9 @@ constexpr int OFFBITS = 11;  // list entry: neighbour index (0..26) << 11 | offs
 constexpr uint32_t OFFMASK = (1u << OFFBITS) - 1u;
 
 struct PairSmem {
-  float4* tso;      // [MAXLOC * 27] first slot (bits), displacement of the neighbour origin x, y, z
-  uint32_t* tcnt;   // [MAXLOC * 27] particles in the neighbour cell
+  float4* tso;      // [MAXLOC * 27] first slot (bits), displacement of the neighbour block origin x, y, z
+  uint32_t* tcnt;   // [MAXLOC * 27] particles in the neighbour run
+  int* tn;          // [MAXLOC] neighbour runs of each local cell
   float* tab;       // [8 * 16] type-pair tables: a, gamma, sigma/sqrt(dt), s_R, kappa[0..3]
   uint16_t* list;   // [lcap][NT]
 };
@@ -136,7 +137,8 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
   sm.tso = (float4*)smem_raw;
   sm.tcnt = (uint32_t*)(smem_raw + (size_t)MAXLOC * 27 * 16);
   sm.tab = (float*)(smem_raw + (size_t)MAXLOC * 27 * 20);
-  sm.list = (uint16_t*)(smem_raw + (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4);
+  sm.tn = (int*)(smem_raw + (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4);
+  sm.list = (uint16_t*)(smem_raw + (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4 + MAXLOC * 4);
 
   const int64_t n = A.n;
   const int64_t i0 = (int64_t)blockIdx.x * NT, i = i0 + t;
@@ -174,26 +176,29 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
   for (uint32_t rb = r_first; rb <= r_last; rb += MAXLOC) {
     const int nloc = (int)min((uint32_t)MAXLOC, r_last - rb + 1u);
     __syncthreads();
-    // ---- neighbour table of the cells rb .. rb + nloc - 1
+    // ---- neighbour runs of the cells rb .. rb + nloc - 1 (static segments + this step's cell table)
     for (int idx = t; idx < nloc * 27; idx += NT) {
-      const int lc = idx / 27, c = idx - lc * 27;
-      const uint32_t pc = __ldg(&A.rank_cell[rb + lc]);
-      const int d[3] = {c % 3 - 1, (c / 3) % 3 - 1, c / 9 - 1};
-      int cc[3] = {(int)(pc & 1023u) + d[0], (int)((pc >> 10) & 1023u) + d[1], (int)(pc >> 20) + d[2]};
-      float off[3];
+      const int lc = idx / 27, k = idx - lc * 27;
+      const uint32_t r = rb + lc;
+      const uint32_t o0 = __ldg(&A.seg_off[r]), nseg = __ldg(&A.seg_off[r + 1]) - o0;
+      if (k == 0) sm.tn[lc] = (int)nseg;
+      if ((uint32_t)k < nseg) {
+        const uint32_t first = __ldg(&A.seg_first[o0 + k]), meta = __ldg(&A.seg_meta[o0 + k]);
+        const uint32_t pc = __ldg(&A.rank_cell[r]), pn = __ldg(&A.rank_cell[first]);
+        float off[3];
 #pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        float w = 0.0f;
-        if (cc[a] < 0) { cc[a] += P.ncell[a]; w = -1.0f; }
-        else if (cc[a] >= P.ncell[a]) { cc[a] -= P.ncell[a]; w = 1.0f; }
-        off[a] = fmaf(w, P.gap[a], (float)d[a] * P.edge_q[a]);  // origin of the neighbour image - own origin
+        for (int a = 0; a < 3; ++a) {
+          const int ci = (int)((pc >> (10 * a)) & 1022u), cj = (int)((pn >> (10 * a)) & 1022u);  // block coordinates
+          const float w = (float)((int)((meta >> (4 + 2 * a)) & 3u) - 1);
+          // origin of the neighbour block image - own block origin: both terms exact, their sum too (nearby numbers)
+          off[a] = __fadd_rn((float)(cj - ci) * P.edge_q[a], w * P.box[a]);
+        }
+        const uint32_t s0 = __ldg(&A.cell_start[first]), s1 = __ldg(&A.cell_start[first + (meta & 15u)]);
+        uint32_t cnt = s1 - s0;
+        if (cnt > OFFMASK) { cnt = OFFMASK; atomicOr(A.err, TD_ERR_CELL_OVERFLOW); }
+        sm.tso[idx] = make_float4(__uint_as_float(s0), off[0], off[1], off[2]);
+        sm.tcnt[idx] = cnt;
       }
-      const uint32_t rk = __ldg(&A.cell_rank[(cc[2] * P.ncell[1] + cc[1]) * P.ncell[0] + cc[0]]);
-      const uint32_t s0 = __ldg(&A.cell_start[rk]), s1 = __ldg(&A.cell_start[rk + 1]);
-      uint32_t cnt = s1 - s0;
-      if (cnt > OFFMASK) { cnt = OFFMASK; atomicOr(A.err, TD_ERR_CELL_OVERFLOW); }
-      sm.tso[idx] = make_float4(__uint_as_float(s0), off[0], off[1], off[2]);
-      sm.tcnt[idx] = cnt;
     }
     __syncthreads();
     const bool mine = active && ri >= rb && ri - rb < (uint32_t)nloc;
@@ -211,9 +216,11 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
     const int sh = 31 - __clz((int)stride);
     const uint32_t lf32 = (uint32_t)__cvta_generic_to_shared(lfront), lb32 = (uint32_t)__cvta_generic_to_shared(lback);
     uint32_t pa = lf32, pb = lb32;
+    const int myn = mine ? sm.tn[me.lc27 / 27] : 0;
+    const int clast = __reduce_max_sync(0xffffffffu, myn) - 1;  // warp-uniform number of neighbour runs - 1
     int c = 0;
     float4 te = sm.tso[me.lc27];
-    uint32_t e = 0, ecnt = mine ? sm.tcnt[me.lc27] : 0u;
+    uint32_t e = 0, ecnt = 0 < myn ? sm.tcnt[me.lc27] : 0u;
     while (true) {
       {
         const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x) - ((uint32_t)c << OFFBITS);  // by entry
@@ -243,7 +250,7 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
       const bool anymore = __any_sync(0xffffffffu, more);
       const int nA = (int)((pa - lf32) >> sh), nB = (int)((lb32 - pb) >> sh);
       int dA, dB;
-      if ((!anymore && c == 26) || __any_sync(0xffffffffu, more && pa > pb)) {
+      if ((!anymore && c >= clast) || __any_sync(0xffffffffu, more && pa > pb)) {
         dA = nA; dB = nB;
       } else {
         const int mA = __reduce_min_sync(0xffffffffu, mine ? nA : 0x7fffffff);
@@ -258,11 +265,11 @@ __global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevPara
         pb += (uint32_t)dB * stride;
       }
       if (!anymore) {
-        if (c == 26) break;
+        if (c >= clast) break;
         ++c;
         te = sm.tso[me.lc27 + c];
         e = (uint32_t)c << OFFBITS;
-        ecnt = e + (mine ? sm.tcnt[me.lc27 + c] : 0u);
+        ecnt = e + (c < myn ? sm.tcnt[me.lc27 + c] : 0u);
       }
     }
     if (mine) {
@@ -296,7 +303,7 @@ int launch_s(const DevParams& P, const PairArgs& A, int nblk, int nthreads, size
 }  // namespace
 
 size_t td_pair_smem_bytes(int lcap, int nthreads) {
-  return (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4 + (size_t)lcap * nthreads * 2;
+  return (size_t)MAXLOC * 27 * 20 + 8 * 16 * 4 + MAXLOC * 4 + (size_t)lcap * nthreads * 2;
 }
 
 int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st) {
