@@ -5,24 +5,28 @@
 // Every pair is evaluated on both sides; there are no atomics, so per-particle sums are deterministic.
 //
 // Design (B200).  One thread owns one particle of the cell-sorted order; a CTA owns NT consecutive slots, i.e. a
-// compact blob of ~NT/13 Morton-consecutive cells.  Nothing is staged: the candidate positions are read through
-// L1 (lanes of one cell read the same address), in coordinates RELATIVE to their cell origin (PairRec::P4), so
-// that the inner loops have no minimum-image arithmetic and fp32 differences are exact to ~2^-22 at any box size.
-//   prologue  the CTA builds, for each of its cells, the table of the 27 neighbour cells: first slot, particle
-//             count and the displacement of the neighbour's origin (periodic image resolved here).
-//   phase 1   each thread scans the 27 cells and appends the hits, branch-free, to a private two-ended list of
-//             16-bit entries (neighbour cell << 11 | offset) in shared memory: front r < min(r_c, r_cc), back the
-//             ring up to max(r_c, r_cc).  86 % of the candidates are rejected here for ~13 instructions each.
-//   phase 2   runs the expensive per-pair work (Philox-4x32-10, Box-Muller, weights) over the dense lists, two
-//             entries per iteration for instruction-level parallelism.
-// Shared memory per thread is ~210 B, so 32 warps per SM are resident (the first version staged whole halos and
-// ran 8).
+// compact blob of ~NT/13 Morton-consecutive cells.  Nothing is staged: candidate positions are read through L1
+// (lanes of one cell read the same address), in coordinates RELATIVE to the origin of their 2x2x2 cell block
+// (PairRec::P4), so that the inner loops have no minimum-image arithmetic and fp32 differences are exact to
+// ~2^-22 at any box size.
+//   prologue  the CTA resolves, for each of its cells, the static neighbour runs (PairArgs::seg_*: the 27
+//             neighbour cells merged into ~14 runs of rank-consecutive cells, longest first) against this step's
+//             cell table: first slot, particle count, displacement of the run's block origin (periodic image).
+//   scan      each thread walks its runs and pushes the hits, branch-free, onto a private two-ended stack of 16-bit
+//             entries (run << 11 | offset) in shared memory: front r < min(r_c, r_cc), back the ring up to
+//             max(r_c, r_cc).  85 % of the candidates are rejected here for ~14 instructions each.
+//   drain     after every run the warp pops the largest multiple of 4 (front) / 8 (back) entries that EVERY lane
+//             owns and evaluates them (Philox-4x32-10, Box-Muller, weights), two entries per iteration for
+//             instruction-level parallelism, so the expensive loops run with all lanes busy; a full stack or the
+//             end of the stencil drains everything.
+// Shared memory per thread is ~240 B (24 warps per SM at 80 registers); the first version staged whole halos, ran
+// 8 warps per SM and took 4.8x longer.
 #include "common.cuh"
 
 namespace {
 
 constexpr int MAXLOC = 32;   // cells per table chunk
-constexpr int OFFBITS = 11;  // list entry: neighbour index (0..26) << 11 | offset inside the neighbour cell
+constexpr int OFFBITS = 11;  // list entry: neighbour run (0..26) << 11 | offset inside the run
 constexpr uint32_t OFFMASK = (1u << OFFBITS) - 1u;
 
 struct PairSmem {
