@@ -198,6 +198,18 @@ def cpu_baseline(c: int, seconds: float = 20.0) -> dict:
 
 
 # --------------------------------------------------------------------------------------------------------------
+def aggregate(dist, device, ms, ms_e2e, n):
+    """Replicas only: whole-job figures = particles summed over ranks / the slowest rank's device time."""
+    import torch
+    if dist is None:
+        return ms, ms_e2e, float(n)
+    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    m = torch.tensor([float(n)], dtype=torch.float64, device=device)
+    dist.all_reduce(m, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), float(m[0])
+
+
 def run_ours(args) -> dict | None:
     import torch
     import paper_1611_06163_b200 as T
@@ -285,14 +297,7 @@ def run_ours(args) -> dict | None:
     ms_e2e = max(a.elapsed_time(b), 1e3 * (time.perf_counter() - t0))
     barrier()
 
-    tmax, temax, ntot = ms, ms_e2e, float(n)
-    if dist is not None:
-        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tmax, temax = float(t[0]), float(t[1])
-        t = torch.tensor([float(n)], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        ntot = float(t[0])
+    tmax, temax, ntot = aggregate(dist, f"cuda:{local}", ms, ms_e2e, n)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -309,14 +314,13 @@ def run_ours(args) -> dict | None:
     ach = bud["flop"] / (pair_ms * 1e-3) / 1e12
     issue_peak = SM_COUNT * LANES_PER_SM * SM_MAX_MHZ * 1e6  # lane-instructions / s
     kernel_ms = {k: v["ms"] / max(K, 1) for k, v in tim.items()}
-    step_ms_sum = sum(kernel_ms.values())
     pair_hbm_bytes = n * (32 + 16 + 16 + 8 * max(S - 1, 0))  # pos+vel (+lo, meta) in, F4 (+Qx) out, per particle
     roof = {
         "kernel": "k_pair", "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
         "frac": ach / FP32_PEAK_TFLOPS,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md §7); not in MEASURED_PEAKS.json",
         "traffic": None,
-        "ms_per_launch": pair_ms, "flop_per_launch": bud["flop"], "share_of_step": kernel_ms["pair"] / step_ms_sum,
+        "ms_per_launch": pair_ms, "flop_per_launch": bud["flop"], "share_of_step": kernel_ms["pair"] / (ms / max(K, 1)),
         "issue_slot_frac": bud["lane_instr"] / (pair_ms * 1e-3) / issue_peak,
         "hbm_gbs_algorithmic": pair_hbm_bytes / (pair_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
         "hbm_peak_source": hbm_src, "census": cen,
@@ -336,6 +340,7 @@ def run_ours(args) -> dict | None:
                         "re-evaluation set_state implies, tdpd_get_state (device -> pinned host)"},
         "gpu_launches": int(launches), "clocks": clk, "roofline": roof,
         "kernel_ms_per_step": kernel_ms,
+        "kernel_ms_note": "CUDA-event time per class per step on its own stream; membrane runs on the second stream concurrently with pair, so its figure includes the time it shares the SMs with the pair kernel",
     }
     if not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(c)
