@@ -27,46 +27,63 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_hist(const uint32_t* __restric
   hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
 }
 
-// exclusive scan of hist[0..total) by one CTA of 1024 threads
-__global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ hist, int64_t total) {
-  __shared__ uint32_t wsum[32];
-  __shared__ uint32_t carry_s;
+// exclusive scan of hist[0..total) in two levels: every CTA scans one chunk of 4096 entries in place and writes the
+// chunk total; k_sort_scan_tops then scans the chunk totals (one CTA); the scatter adds tops[index >> 12]
+constexpr int SCAN_CHUNK = 4096;
+__device__ __forceinline__ uint32_t block_excl_scan_1024(uint32_t tsum, uint32_t* wsum, uint32_t& total) {
   int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  if (threadIdx.x == 0) carry_s = 0;
-  __syncthreads();
-  for (int64_t base = 0; base < total; base += 4096) {
-    int64_t i0 = base + (int64_t)threadIdx.x * 4;
-    uint32_t v[4];
+  uint32_t x = tsum;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = (i0 + k < total) ? hist[i0 + k] : 0u;
-    uint32_t tsum = v[0] + v[1] + v[2] + v[3];
-    uint32_t x = tsum;
+  for (int d = 1; d < 32; d <<= 1) {
+    uint32_t y = __shfl_up_sync(0xffffffffu, x, d);
+    if (lane >= d) x += y;
+  }
+  if (lane == 31) wsum[w] = x;
+  __syncthreads();
+  if (w == 0) {
+    uint32_t s = wsum[lane];
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-      uint32_t y = __shfl_up_sync(0xffffffffu, x, d);
-      if (lane >= d) x += y;
+      uint32_t y = __shfl_up_sync(0xffffffffu, s, d);
+      if (lane >= d) s += y;
     }
-    if (lane == 31) wsum[w] = x;
-    __syncthreads();
-    if (w == 0) {
-      uint32_t s = wsum[lane];
+    wsum[lane] = s;  // inclusive over warps
+  }
+  __syncthreads();
+  total = wsum[31];
+  return (w ? wsum[w - 1] : 0u) + (x - tsum);
+}
+
+__global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ hist, int64_t total,
+                                                    uint32_t* __restrict__ tops) {
+  __shared__ uint32_t wsum[32];
+  int64_t i0 = (int64_t)blockIdx.x * SCAN_CHUNK + (int64_t)threadIdx.x * 4;
+  uint32_t v[4];
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        uint32_t y = __shfl_up_sync(0xffffffffu, s, d);
-        if (lane >= d) s += y;
-      }
-      wsum[lane] = s;  // inclusive over warps
-    }
-    __syncthreads();
+  for (int k = 0; k < 4; ++k) v[k] = (i0 + k < total) ? hist[i0 + k] : 0u;
+  uint32_t sum;
+  uint32_t excl = block_excl_scan_1024(v[0] + v[1] + v[2] + v[3], wsum, sum);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    if (i0 + k < total) hist[i0 + k] = excl;
+    excl += v[k];
+  }
+  if (threadIdx.x == 0) tops[blockIdx.x] = sum;
+}
+
+__global__ void __launch_bounds__(1024) k_sort_scan_tops(uint32_t* __restrict__ tops, int nchunk) {
+  __shared__ uint32_t wsum[32];
+  __shared__ uint32_t carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < nchunk; base += 1024) {
+    int i = base + threadIdx.x;
+    uint32_t v = i < nchunk ? tops[i] : 0u, sum;
+    uint32_t excl = block_excl_scan_1024(v, wsum, sum);
     uint32_t carry = carry_s;
-    uint32_t excl = carry + (w ? wsum[w - 1] : 0u) + (x - tsum);
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      if (i0 + k < total) hist[i0 + k] = excl;
-      excl += v[k];
-    }
+    if (i < nchunk) tops[i] = carry + excl;
     __syncthreads();
-    if (threadIdx.x == 0) carry_s = carry + wsum[31];
+    if (threadIdx.x == 0) carry_s = carry + sum;
     __syncthreads();
   }
 }
@@ -77,7 +94,7 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
                                                           const uint32_t* __restrict__ vin,
                                                           uint32_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                           int64_t n, int shift, const uint32_t* __restrict__ hist,
-                                                          int nblk) {
+                                                          int nblk, const uint32_t* __restrict__ tops) {
   __shared__ uint32_t wbase[SORT_NT / 32][NBIN];
   int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int k = threadIdx.x; k < (SORT_NT / 32) * NBIN; k += SORT_NT) (&wbase[0][0])[k] = 0;
@@ -93,7 +110,8 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
   __syncthreads();
   {  // per bin: counts -> exclusive prefix over warps + global base
     int b = threadIdx.x;
-    uint32_t run = hist[(int64_t)b * nblk + blockIdx.x];
+    const int64_t hi = (int64_t)b * nblk + blockIdx.x;
+    uint32_t run = hist[hi] + tops[hi / SCAN_CHUNK];
 #pragma unroll
     for (int ww = 0; ww < SORT_NT / 32; ++ww) {
       uint32_t c = wbase[ww][b];
@@ -168,7 +186,8 @@ int td_sort_passes(int key_bits) { return key_bits <= 0 ? 1 : (key_bits + RB - 1
 size_t td_sort_scratch_bytes(int64_t n) {
   int64_t nblk = (n + TILE - 1) / TILE;
   if (nblk < 1) nblk = 1;
-  return (size_t)nblk * NBIN * sizeof(uint32_t);
+  size_t nh = (size_t)nblk * NBIN;
+  return (nh + (nh + SCAN_CHUNK - 1) / SCAN_CHUNK + 64) * sizeof(uint32_t);
 }
 
 int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits, void* scratch, cudaStream_t st,
@@ -177,15 +196,19 @@ int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits
   if (n == 0) return side;
   int nblk = (int)((n + TILE - 1) / TILE);
   uint32_t* hist = (uint32_t*)scratch;
+  const int64_t nh = (int64_t)nblk * NBIN;
+  const int nchunk = (int)((nh + SCAN_CHUNK - 1) / SCAN_CHUNK);
+  uint32_t* tops = hist + nh;
   int passes = td_sort_passes(key_bits);
   for (int p = 0; p < passes; ++p) {
     int shift = p * RB;
     k_sort_hist<<<nblk, SORT_NT, 0, st>>>(keys[side], n, shift, hist, nblk);
-    k_sort_scan<<<1, 1024, 0, st>>>(hist, (int64_t)nblk * NBIN);
+    k_sort_scan<<<nchunk, 1024, 0, st>>>(hist, nh, tops);
+    k_sort_scan_tops<<<1, 1024, 0, st>>>(tops, nchunk);
     k_sort_scatter<<<nblk, SORT_NT, 0, st>>>(keys[side], vals[side], keys[side ^ 1], vals[side ^ 1], n, shift, hist,
-                                              nblk);
+                                              nblk, tops);
     side ^= 1;
-    if (n_launches) *n_launches += 3;
+    if (n_launches) *n_launches += 4;
   }
   return side;
 }

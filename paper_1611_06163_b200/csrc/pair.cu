@@ -23,9 +23,12 @@
 // 8 warps per SM and took 4.8x longer.
 #include "common.cuh"
 
+#ifndef TD_PAIR_MINB
+#define TD_PAIR_MINB 3
+#endif
 namespace {
 
-constexpr int MAXLOC = 32;   // cells per table chunk
+constexpr int MAXLOC = 24;   // cells per table chunk
 constexpr int OFFBITS = 11;  // list entry: neighbour run (0..26) << 11 | offset inside the run
 constexpr uint32_t OFFMASK = (1u << OFFBITS) - 1u;
 
@@ -133,7 +136,7 @@ __device__ __forceinline__ void eval_list(const DevParams& P, const PairArgs& A,
 
 // RING: 1 = r_cc >= r_c (ring entries are flux-only), 2 = r_c > r_cc (ring entries are force-only)
 template <int S, bool RANDFLUX, bool FASTW, int RING>
-__global__ void __launch_bounds__(256, 3) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
+__global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int NT = blockDim.x, t = threadIdx.x;
   const int lcap = A.lcap;
