@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtdpd.so")
 SOURCES = ["api.cu", "integrate.cu", "binning.cu", "pair.cu", "membrane.cu", "debug.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = (["-DTD_PAIR_MINB=" + os.environ["TD_PAIR_MINB"]] if "TD_PAIR_MINB" in os.environ else []) + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
+FLAGS = [f"-D{k}={v}" for k, v in os.environ.items() if k.startswith("TD_PAIR_")] + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
 def _stale() -> bool:

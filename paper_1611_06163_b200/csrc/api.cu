@@ -672,7 +672,7 @@ int eval_forces(tdpd_sim* s) {
   {
     Scope t(s, 3, s->sA);
     PairArgs A;
-    A.rec = s->rec; A.vel = s->st[c].vel; A.keys = s->keys_sorted;
+    A.rec = s->rec; A.vel = s->st[c].vel; A.pos = s->st[c].pos; A.lo = s->st[c].lo; A.keys = s->keys_sorted;
     A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
     A.seg_off = s->seg_off_d; A.seg_first = s->seg_first_d; A.seg_meta = s->seg_meta_d;
     A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step = (uint32_t)s->step; A.lcap = s->lcap; A.err = s->err_d;

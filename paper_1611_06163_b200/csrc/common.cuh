@@ -126,6 +126,8 @@ struct PairRec {
 struct PairArgs {
   PairRec rec;
   const float4* vel;           // vx, vy, vz, C_0 (SortedState::vel)
+  const float4* pos;           // hi words of the positions (SortedState::pos)
+  const float4* lo;            // low words (SortedState::lo)
   const uint32_t* keys;        // [n] Morton rank of the cell of each slot (sorted)
   const uint32_t* cell_start;  // [ncell + 1] by Morton rank
   const uint32_t* cell_rank;   // [ncell] x-fastest linear cell -> Morton rank

@@ -23,12 +23,19 @@
 // 8 warps per SM and took 4.8x longer.
 #include "common.cuh"
 
+#ifndef TD_PAIR_MAXLOC
+#define TD_PAIR_MAXLOC 32
+#endif
+#ifndef TD_PAIR_UNROLL
+#define TD_PAIR_UNROLL 4
+#endif
 #ifndef TD_PAIR_MINB
 #define TD_PAIR_MINB 3
 #endif
 namespace {
 
-constexpr int MAXLOC = 24;   // cells per table chunk
+constexpr int MAXLOC = TD_PAIR_MAXLOC;   // cells per table chunk
+constexpr int SCAN_UNROLL = TD_PAIR_UNROLL;
 constexpr int OFFBITS = 11;  // list entry: neighbour run (0..26) << 11 | offset inside the run
 constexpr uint32_t OFFMASK = (1u << OFFBITS) - 1u;
 
@@ -107,7 +114,16 @@ __device__ __forceinline__ void pair_eval(const DevParams& P, const PairArgs& A,
   }
   if (FORCE) {
     const float4 vj = __ldg(&A.vel[j]);
-    const float wc = fmaxf(1.0f - r * P.inv_rc, 0.0f);
+    // w_c = 1 - r/r_c enters the random force as w_c^s with s < 1 (sqrt for s = 1/2), which is singular at the
+    // cutoff: an fp32 error of 1e-7 in r becomes 3e-4 in sqrt(w_c) and 0.03 in the force.  The numerator
+    // r_c^2 - r^2 is therefore formed in fp64 from the block-relative coordinates (exact images of the positions
+    // whenever the low words are zero, i.e. after load / set_state; rounded to 2^-24 otherwise) and the exact block
+    // displacement: w_c = (r_c^2 - r^2) / (r_c (r_c + r)), strict r < r_c as in O2.  14 % of the entries come here.
+    const double ex = ((double)me.x - (double)te.y) - (double)pj.x, ey = ((double)me.y - (double)te.z) - (double)pj.y,
+                 ez = ((double)me.z - (double)te.w) - (double)pj.z;
+    const double rc = (double)P.r_c;
+    const float num = (float)(rc * rc - (ex * ex + ey * ey + ez * ez));
+    const float wc = fmaxf(num, 0.0f) * __frcp_rn(P.r_c * (P.r_c + r));
     float wR, wD;
     if (FASTW) { wR = td_sqrt_approx(wc); wD = wc; }
     else { wR = td_pow_w(wc, sm.tab[3 * 16 + tt]); wD = wR * wR; }
@@ -176,7 +192,9 @@ __global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constan
 #pragma unroll
     for (int s = 0; s < TD_S; ++s) sm.tab[(4 + s) * 16 + k] = P.kappa[s][k];
   }
-  const float rin2 = fminf(P.rc2, P.rcc2), rout2 = P.rcut2;
+  // list thresholds, inflated by 1e-6 so that no pair inside a cutoff is lost to fp32 rounding of r^2; the
+  // weights themselves vanish exactly at the true cutoffs (exact numerator for w_c, clamp for w_cc)
+  const float rin2 = fminf(P.rc2, P.rcc2) * 1.000001f, rout2 = P.rcut2 * 1.000001f;
   uint16_t* const lfront = sm.list + t;
   uint16_t* const lback = sm.list + (size_t)(lcap - 1) * NT + t;
 
@@ -234,7 +252,7 @@ __global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constan
         const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
         const uint32_t room = (uint32_t)(((int)(pb - pa) >> sh) + 1);  // free entries (pa <= pb + stride always)
         const uint32_t eend = min(ecnt, e + room);
-#pragma unroll 4
+#pragma unroll SCAN_UNROLL
         for (; e < eend; ++e) {
           const float4 pj = __ldg(&src[e]);
           const float dx = xs - pj.x, dy = ys - pj.y, dz = zs - pj.z;

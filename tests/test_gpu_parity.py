@@ -278,3 +278,43 @@ def test_edge_cases(T):
     with pytest.raises(T.TdpdError):
         s.add_rbc_mesh(np.zeros((4, 3), np.float32), None, None, np.array([[0, 1, 2], [0, 2, 3]], np.int32),
                        W.rbc_params())          # open mesh
+
+
+# ---------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times (automatic pair_threads / list_cap)
+@pytest.mark.parametrize("c", [2, 3, 4, 5])
+def test_full_size_config_one_step_forces(T, orc, c):
+    w = W.config(c)
+    sim = T.Simulation.from_workload(w)
+    o = orc.Oracle.from_workload(w)
+    o.compute_forces(0)
+    check_forces(sim, o, label=f"config{c} full size, step 0")
+    if w.rbcs:
+        gs, ost = sim.rbc_stats(), o.rbc_stats()
+        assert np.allclose(gs["area"], ost["area"], rtol=2e-6) and np.allclose(gs["volume"], ost["volume"], rtol=2e-6)
+    # the census of the whole system is bit-exact as well (cells, neighbour counts, neighbour id checksums)
+    if c <= 3:   # (the oracle's census is the slow part: minutes beyond config 3)
+        oc, gc = o.neighbor_census(), sim.debug_neighbor_census()
+        for k in ("n_rc", "n_rcc", "xor_rc", "xor_rcc"):
+            assert np.array_equal(gc[k], oc[k]), k
+
+
+@pytest.mark.parametrize("c", [2, 3])
+def test_full_size_config_100_steps_positions_and_invariants(T, orc, c):
+    w = W.config(c)
+    sim = T.Simulation.from_workload(w)
+    o = orc.Oracle.from_workload(w)
+    g0 = sim.get_state()
+    sim.step(100)
+    o.step(100)
+    g, os_ = sim.get_state(), o.get_state()
+    d = min_image_diff(g["pos"], os_["pos"], w.params["box"])
+    assert np.abs(d).max() <= 1e-3 * float(w.params["r_c"]), np.abs(d).max()
+    # invariants on the GPU side: total concentration conserved; momentum changes only by the body force
+    c0, c1 = g0["conc"].astype(np.float64).sum(), g["conc"].astype(np.float64).sum()
+    assert abs(c1 - c0) <= 2e-5 * abs(c0)
+    p_g, p_o = g["vel"].astype(np.float64).sum(0), os_["vel"].sum(0)
+    assert np.abs(p_g - p_o).max() <= 2e-5 * len(d) ** 0.5 * 100
+    if w.rbcs:
+        st = sim.rbc_stats()
+        assert np.all(np.abs(st["area"] / st["A0"] - 1) < 5e-3) and np.all(np.abs(st["volume"] / st["V0"] - 1) < 5e-3)
