@@ -228,7 +228,7 @@ def run_ours(args) -> dict | None:
 
     c = args.config
     w = workload(c, rank)
-    sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap)
+    sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap, pair_split=args.pair_split)
     n, S = sim.n, sim.ns
     K, Wm = args.steps, max(3, args.warmup)
     state_bytes = n * (16 * 3 + 4 * max(S - 1, 0))
@@ -357,6 +357,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--pair-threads", type=int, default=0, help="pair-kernel CTA size override (tuning)")
+    ap.add_argument("--pair-split", type=int, default=0, help="pair-kernel threads per particle override (tuning)")
     ap.add_argument("--list-cap", type=int, default=0, help="pair-kernel list capacity override (tuning)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()

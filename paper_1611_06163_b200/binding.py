@@ -113,7 +113,7 @@ def load_library() -> C.CDLL:
     L.tdpd_get_timing.argtypes = [vp, vp, vp]
     L.tdpd_launch_count.argtypes = [vp]
     L.tdpd_launch_count.restype = i64
-    L.tdpd_set_tuning.argtypes = [vp, i32, i32]
+    L.tdpd_set_tuning.argtypes = [vp, i32, i32, i32]
     L.tdpd_last_error.argtypes = [vp]
     L.tdpd_last_error.restype = C.c_char_p
     L.tdpd_destroy.argtypes = [vp]
@@ -134,7 +134,8 @@ def _f32(a):
 class Simulation:
     """One tDPD + RBC simulation on one GPU.  Methods mirror the C ABI one to one."""
 
-    def __init__(self, params: dict, device: int = 0, pair_threads: int = 0, list_cap: int = 0):
+    def __init__(self, params: dict, device: int = 0, pair_threads: int = 0, list_cap: int = 0,
+                 pair_split: int = 0):
         import torch
 
         self.L = load_library()
@@ -156,8 +157,8 @@ class Simulation:
         self.h = h
         self.workspace = None
         self._ntri = []
-        if pair_threads or list_cap:
-            self._ck(self.L.tdpd_set_tuning(self.h, pair_threads, list_cap))
+        if pair_threads or list_cap or pair_split:
+            self._ck(self.L.tdpd_set_tuning(self.h, pair_threads, list_cap, pair_split))
 
     def _ck(self, rc):
         if rc != OK:

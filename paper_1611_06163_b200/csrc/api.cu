@@ -55,7 +55,7 @@ struct tdpd_sim {
   int key_bits = 0;
   std::vector<uint32_t> cell_rank, rank_cell;
   std::vector<uint32_t> seg_off, seg_first, seg_meta;  // static neighbour runs of every cell (PairArgs)
-  int pair_nt = 256, lcap = 72, tune_nt = 0, tune_lcap = 0;
+  int pair_nt = 256, lcap = 72, pair_split = 1, tune_nt = 0, tune_lcap = 0, tune_split = 0;
   PairRec rec = {nullptr, nullptr, nullptr};
   uint32_t* keys_sorted = nullptr;
   int mem_nchunk = 1, mem_nt = 256, max_nv = 0;
@@ -433,10 +433,13 @@ static void build_grid(tdpd_sim* s) {
   {
     double rcut = std::max(s->prm.r_c, s->prm.r_cc);
     double mn = 4.18879 * rcut * rcut * rcut * (double)s->n / ((double)s->prm.box[0] * s->prm.box[1] * s->prm.box[2]);
-    int lc = ((int)(mn * 1.4) + 8 + 1) / 2 * 2;
+    // sub-wave systems (fewer particles than the GPU has thread slots): several threads per particle
+    int split = s->n >= 60000 ? 1 : (s->n >= 20000 ? 4 : 16);
+    s->pair_split = s->tune_split ? s->tune_split : split;
+    int lc = ((int)(mn * 1.4 / s->pair_split) + 8 + 1) / 2 * 2;
     s->lcap = s->tune_lcap ? s->tune_lcap : std::min(160, std::max(16, lc));
-    int nt = s->n >= 148 * 8 * 256 ? 256 : (s->n >= 148 * 8 * 128 ? 128 : 64);
-    s->pair_nt = s->tune_nt ? s->tune_nt : nt;
+    s->pair_nt = s->tune_nt ? s->tune_nt : (s->pair_split == 1 ? 256 : 128);
+    if (s->pair_nt < s->pair_split) s->pair_nt = s->pair_split;
   }
   // membrane kernel: CTAs per membrane so that small suspensions still fill the machine
   int M = (int)s->rbcs.size();
@@ -676,7 +679,7 @@ int eval_forces(tdpd_sim* s) {
     A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
     A.seg_off = s->seg_off_d; A.seg_first = s->seg_first_d; A.seg_meta = s->seg_meta_d;
     A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step = (uint32_t)s->step; A.lcap = s->lcap; A.err = s->err_d;
-    int rc = td_launch_pair(s->dp, A, s->pair_nt, s->sA);
+    int rc = td_launch_pair(s->dp, A, s->pair_nt, s->pair_split, s->sA);
     if (rc) return fail(s, TDPD_ECUDA, std::string("pair kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
     s->launches += 1; s->timers[3].launches += 1;
   }
@@ -972,13 +975,16 @@ extern "C" int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], dou
 
 extern "C" int64_t tdpd_launch_count(const tdpd_sim* s) { return s ? s->launches : 0; }
 
-extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap) {
+extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap, int32_t pair_split) {
   if (!s) return TDPD_EINVAL;
   if (s->finalized) return fail(s, TDPD_ESTATE, "tuning must be set before tdpd_set_workspace");
   if (pair_threads != 0 && pair_threads != 32 && pair_threads != 64 && pair_threads != 128 && pair_threads != 256)
     return fail(s, TDPD_EINVAL, "pair_threads must be 0, 32, 64, 128 or 256");
   if (list_cap != 0 && (list_cap < 4 || list_cap > 400)) return fail(s, TDPD_EINVAL, "list_cap must be 0 or 4..400");
+  if (pair_split != 0 && pair_split != 1 && pair_split != 4 && pair_split != 16)
+    return fail(s, TDPD_EINVAL, "pair_split must be 0, 1, 4 or 16");
   s->tune_nt = pair_threads;
+  s->tune_split = pair_split;
   s->tune_lcap = list_cap;
   return TDPD_OK;
 }

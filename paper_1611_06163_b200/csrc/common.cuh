@@ -184,6 +184,10 @@ struct MembraneArgs {
 
 enum { TD_ERR_CELL_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4 };
 
+#ifndef TD_PAIR_MAXLOC
+#define TD_PAIR_MAXLOC 32  // cells per neighbour-table chunk of the pair kernel
+#endif
+
 // ---- launchers (each .cu exposes host functions; all launches are asynchronous on `st`) -------------------
 void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
                          const uint32_t* cell_rank, cudaStream_t st);
@@ -200,7 +204,7 @@ int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits
 void td_launch_reorder(const DevParams& P, const SortedState& src, const SortedState& dst, const PairRec& rec,
                        const uint32_t* keys, const uint32_t* vals, const uint32_t* rank_cell, int64_t n,
                        uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, cudaStream_t st);
-int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st);
+int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, int split, cudaStream_t st);
 size_t td_pair_smem_bytes(int lcap, int nthreads);
 int td_launch_membrane(const DevParams& P, const MembraneArgs& A, int n_rbc, int max_nv, int nthreads,
                        cudaStream_t st);

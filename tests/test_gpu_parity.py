@@ -107,14 +107,15 @@ def test_config1_one_step_forces(T, orc):
     check_forces(sim, o, label="config1 step 3")
 
 
-@pytest.mark.parametrize("nt,cap", [(32, 4), (64, 16), (128, 0), (256, 0), (256, 7)])
-def test_pair_launch_shapes_agree(T, orc, nt, cap):
+@pytest.mark.parametrize("nt,cap,split", [(32, 4, 1), (64, 16, 1), (128, 0, 1), (256, 0, 1), (256, 7, 1), (128, 0, 4),
+                                          (64, 4, 4), (256, 0, 16), (32, 5, 16)])
+def test_pair_launch_shapes_agree(T, orc, nt, cap, split):
     # 8 x 6 x 5 cells (not powers of two: holes in the Morton rank range); tiny list caps force mid-scan flushes
     w = W.make_fluid("t", (13, 11, 8), 4.0, seed=21)
-    sim = T.Simulation.from_workload(w, pair_threads=nt, list_cap=cap)
+    sim = T.Simulation.from_workload(w, pair_threads=nt, list_cap=cap, pair_split=split)
     o = orc.Oracle.from_workload(w)
     o.compute_forces(0)
-    check_forces(sim, o, label=f"pair_threads {nt} list_cap {cap}")
+    check_forces(sim, o, label=f"pair_threads {nt} list_cap {cap} pair_split {split}")
 
 
 def test_random_flux_off_and_general_exponents(T, orc):
@@ -318,3 +319,36 @@ def test_full_size_config_100_steps_positions_and_invariants(T, orc, c):
     if w.rbcs:
         st = sim.rbc_stats()
         assert np.all(np.abs(st["area"] / st["A0"] - 1) < 5e-3) and np.all(np.abs(st["volume"] / st["V0"] - 1) < 5e-3)
+
+
+def test_pairs_at_the_force_cutoff(T, orc):
+    """w_R = (1 - r/r_c)^(1/2) is singular at r = r_c: pairs within a few fp32 ulps of the cutoff (config 5 has
+    some at every step) must still agree with the oracle, and pairs just outside must feel no force."""
+    p = W.fluid_params((16, 16, 16), 4.0, seed=77)
+    base = np.array([[2, 2, 2], [6, 2, 2], [10, 2, 2], [2, 6, 2], [6, 6, 2], [10, 6, 2], [2, 10, 9], [6, 10, 9]],
+                    np.float32)
+    one = np.float32(1.0)
+    seps = [np.nextafter(one, np.float32(0)), one - np.float32(3e-7), one - np.float32(1e-6), one - np.float32(1e-5),
+            one, np.nextafter(one, np.float32(2)), one + np.float32(1e-6), one - np.float32(1e-3)]
+    dirs = np.array([[1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 0, 0], [0, -1, 0], [0, 0, -1], [-1, 0, 0], [0, 1, 0]],
+                    np.float32)
+    pos = np.concatenate([base, base + dirs * np.array(seps, np.float32)[:, None]]).astype(np.float32)
+    rng = np.random.Generator(np.random.PCG64(3))
+    vel = rng.standard_normal(pos.shape).astype(np.float32)
+    conc = rng.random((len(pos), 1)).astype(np.float32)
+    sim = T.Simulation(p)
+    sim.load_particles(pos, vel, None, conc)
+    sim.finalize()
+    o = orc.Oracle(p)
+    o.load_particles(pos, vel, None, conc)
+    o.compute_forces(0)
+    g, r = sim.get_state(), o.get_state()
+    err = np.abs(g["force"] - r["force"]).max(axis=1)
+    assert err.max() <= 1e-4 * 20.0, err        # 20 = a typical RMS force of the configs
+    r_act = np.linalg.norm(pos[8:].astype(np.float64) - pos[:8].astype(np.float64), axis=1)  # of the fp32 positions
+    assert (r_act < 1.0).sum() >= 4 and (r_act >= 1.0).sum() >= 2
+    for k in range(8):
+        if r_act[k] >= 1.0:
+            assert np.all(g["force"][k] == 0) and np.all(r["force"][k] == 0)
+        else:
+            assert np.any(r["force"][k] != 0) and np.any(g["force"][k] != 0)
