@@ -74,6 +74,11 @@ __device__ __forceinline__ float td_rsqrt_approx(float x) {
   return y;
 }
 
+__device__ __forceinline__ float td_rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ float td_lg2_approx(float x) {
   float y;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));

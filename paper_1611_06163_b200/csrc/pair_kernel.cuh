@@ -124,7 +124,7 @@ __device__ __forceinline__ void pair_eval(const DevParams& P, const PairArgs& A,
                  ez = ((double)me.z - (double)te.w) - (double)pj.z;
     const double rc = (double)P.r_c;
     const float num = (float)(rc * rc - (ex * ex + ey * ey + ez * ez));
-    const float wc = fmaxf(num, 0.0f) * __frcp_rn(P.r_c * (P.r_c + r));
+    const float wc = fmaxf(num, 0.0f) * td_rcp_approx(P.r_c * (P.r_c + r));
     float wR, wD;
     if (FASTW) { wR = td_sqrt_approx(wc); wD = wc; }
     else { wR = td_pow_w(wc, sm.tab[3 * 16 + tt]); wD = wR * wR; }
