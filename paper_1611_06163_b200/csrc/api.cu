@@ -596,7 +596,7 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
     h0.insert(h0.end(), R.h0.begin(), R.h0.end());
     kp.insert(kp.end(), R.kp.begin(), R.kp.end());
     a0t.insert(a0t.end(), R.A0t.begin(), R.A0t.end());
-    D.A0 = (float)R.A0; D.V0 = (float)R.V0;
+    D.A0 = R.A0; D.V0 = R.V0;
     D.kBT_over_p = (float)(kBT / (double)R.rp.p);
     D.inv_x0 = (float)(1.0 / (double)R.rp.x0);
     D.m_pow = R.rp.m; D.gamma_T = R.rp.gamma_T; D.gamma_C = R.rp.gamma_C;

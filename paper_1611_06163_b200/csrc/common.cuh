@@ -113,6 +113,20 @@ __device__ __forceinline__ void td_box_muller(uint32_t xa, uint32_t xb, float& g
   g_sin = R * td_sin_approx(ang);
 }
 
+// full-precision variant (libdevice logf / sincospif, ~1 ulp) for the membrane kernel: bond random forces carry the
+// prefactor sqrt(2 kBT/dt) sqrt(2 gamma_T) ~ 35, so the 1e-5 absolute error of the MUFU path would cost 1e-3 in the
+// force of a vertex; there are only ~4 bonds per membrane vertex, so the cost is nil
+__device__ __forceinline__ void td_box_muller_precise(uint32_t xa, uint32_t xb, float& g_cos, float& g_sin) {
+  const float u = td_uniform(xa);
+  const float t = 1.0f - u;
+  const float q = t < 7.62939453125e-06f ? fmaf(t, t, t + t) : -2.0f * logf(u);
+  const float R = sqrtf(q);
+  float sn, cs;
+  sincospif(2.0f * td_uniform(xb), &sn, &cs);
+  g_cos = R * cs;
+  g_sin = R * sn;
+}
+
 // ---- kernel argument blocks -----------------------------------------------------------------------------
 struct SortedState {   // one side of the ping-pong, cell-sorted order
   float4* pos;     // x, y, z, id (bits)
@@ -167,7 +181,7 @@ struct RbcDev {
   int tmpl;
   int data_off;  // offset of this membrane's h0/kp (per bond) arrays
   int tri_off;   // offset of A0t
-  float A0, V0;
+  double A0, V0;  // fp64: (A - A0) / A0 is multiplied by k_g ~ 2e4, an fp32 A0 alone would cost 1e-3 in beta
   float kBT_over_p, inv_x0, m_pow, gamma_T, gamma_C, k_g, k_l, k_v, k_b, cos_t0, sin_t0;
   float rnd_T, rnd_C;  // sqrt(2 kBT/dt) sqrt(2 gT), sqrt(2 kBT/dt) sqrt(3 gC - gT)/3
 };

@@ -82,8 +82,8 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
     if (chunk == 0) { A.stats[2 * m] = sA; A.stats[2 * m + 1] = sV; }
   }
   __syncthreads();
-  const float beta_g = (float)(-(double)R.k_g * (tot[0] - (double)R.A0) / (double)R.A0);
-  const float beta_v6 = (float)(-(double)R.k_v * (tot[1] - (double)R.V0) / (double)R.V0 / 6.0);
+  const float beta_g = (float)(-(double)R.k_g * (tot[0] - R.A0) / R.A0);
+  const float beta_v6 = (float)(-(double)R.k_v * (tot[1] - R.V0) / R.V0 / 6.0);
 
   // ---- per-vertex forces
   const int CH = (nv + A.nchunk - 1) / A.nchunk;
@@ -116,8 +116,8 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
         uint32_t x0, x1, x2, x3;
         float g0, g1, g2, g3;
         td_philox(lo, hi, A.step, 1u + row, P.key0, P.key1, x0, x1, x2, x3);
-        td_box_muller(x0, x1, g0, g1);
-        td_box_muller(x2, x3, g2, g3);
+        td_box_muller_precise(x0, x1, g0, g1);
+        td_box_muller_precise(x2, x3, g2, g3);
         N[3 * row] = g0; N[3 * row + 1] = g1; N[3 * row + 2] = g2;
       }
       float tr = N[0] + N[4] + N[8];
