@@ -47,8 +47,8 @@ OPS = dict(cand=(8, 7), flux=(8, 7), rflux=(9, 8), force=(28, 21), philox=(0, 70
 
 
 # --------------------------------------------------------------------------------------------------------------
-def workload(c: int, rank: int = 0):
-    w = W.config(c)
+def workload(c: int, rank: int = 0, random_flux: bool = True):
+    w = W.config(c) if random_flux else W.config(c, m_s=0.0)  # m_s = 0: the paper's own setting
     if rank:  # replicas differ only in the random stream
         w.params = dict(w.params, seed=int(w.params["seed"]) + 7919 * rank)
     return w
@@ -227,7 +227,7 @@ def run_ours(args) -> dict | None:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
 
     c = args.config
-    w = workload(c, rank)
+    w = workload(c, rank, args.random_flux == "on")
     sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap, pair_split=args.pair_split)
     n, S = sim.n, sim.ns
     K, Wm = args.steps, max(3, args.warmup)
@@ -359,6 +359,8 @@ def main():
     ap.add_argument("--pair-threads", type=int, default=0, help="pair-kernel CTA size override (tuning)")
     ap.add_argument("--pair-split", type=int, default=0, help="pair-kernel threads per particle override (tuning)")
     ap.add_argument("--list-cap", type=int, default=0, help="pair-kernel list capacity override (tuning)")
+    ap.add_argument("--random-flux", default="on", choices=["on", "off"],
+                    help="off: m_s = 0, the random concentration flux dropped as in the paper (PAPER.md:78)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
