@@ -30,6 +30,9 @@
 #ifndef TD_PAIR_UNROLL
 #define TD_PAIR_UNROLL 4
 #endif
+#ifndef TD_PAIR_ILP
+#define TD_PAIR_ILP 2  // list entries evaluated per iteration
+#endif
 #ifndef TD_PAIR_MINB
 #define TD_PAIR_MINB 3
 #endif
@@ -142,6 +145,10 @@ template <int S, bool RANDFLUX, bool FASTW, int MODE>
 __device__ __forceinline__ void eval_list(const DevParams& P, const PairArgs& A, const PairSmem& sm, const Self& me,
                                           const uint16_t* base, int stride, int cnt, float& fx, float& fy, float& fz,
                                           float* q) {
+#if TD_PAIR_ILP == 1
+  for (int k = 0; k < cnt; ++k)
+    pair_eval<S, RANDFLUX, FASTW, MODE>(P, A, sm, me, base[k * stride], 1.0f, fx, fy, fz, q);
+#else
   for (int k = 0; k < cnt; k += 2) {
     const bool two = k + 1 < cnt;
     const uint32_t e0 = base[k * stride];
@@ -149,6 +156,7 @@ __device__ __forceinline__ void eval_list(const DevParams& P, const PairArgs& A,
     pair_eval<S, RANDFLUX, FASTW, MODE>(P, A, sm, me, e0, 1.0f, fx, fy, fz, q);
     pair_eval<S, RANDFLUX, FASTW, MODE>(P, A, sm, me, e1, two ? 1.0f : 0.0f, fx, fy, fz, q);
   }
+#endif
 }
 
 // RING: 1 = r_cc >= r_c (ring entries are flux-only), 2 = r_c > r_cc (ring entries are force-only)
