@@ -184,7 +184,7 @@ int64_t tdpd_launch_count(const tdpd_sim* s);
 /* Pair-kernel launch knobs (tuning; results are identical up to the fp32 summation order of a particle's
  * neighbours): pair_threads in {32, 64, 128, 256} = threads per CTA, list_cap in 4..400 = entries of the
  * per-thread neighbour list in shared memory (a full list is evaluated early, never overflowed), pair_split in
- * {1, 4, 16} = threads per particle (sub-wave systems); 0 = automatic.  ESTATE after tdpd_set_workspace. */
+ * {1, 2, 4, 16} = threads per particle (sub-wave systems); 0 = automatic.  ESTATE after tdpd_set_workspace. */
 int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap, int32_t pair_split);
 
 const char* tdpd_last_error(const tdpd_sim* s);

@@ -434,11 +434,11 @@ static void build_grid(tdpd_sim* s) {
     double rcut = std::max(s->prm.r_c, s->prm.r_cc);
     double mn = 4.18879 * rcut * rcut * rcut * (double)s->n / ((double)s->prm.box[0] * s->prm.box[1] * s->prm.box[2]);
     // sub-wave systems (fewer particles than the GPU has thread slots): several threads per particle
-    int split = s->n >= 60000 ? 1 : (s->n >= 20000 ? 4 : 16);
+    int split = s->n >= 300000 ? 1 : (s->n >= 20000 ? 2 : 16);
     s->pair_split = s->tune_split ? s->tune_split : split;
     int lc = ((int)(mn * 1.4 / s->pair_split) + 8 + 1) / 2 * 2;
     s->lcap = s->tune_lcap ? s->tune_lcap : std::min(160, std::max(16, lc));
-    s->pair_nt = s->tune_nt ? s->tune_nt : (s->pair_split == 1 ? 256 : 128);
+    s->pair_nt = s->tune_nt ? s->tune_nt : (s->pair_split <= 2 ? 256 : 128);
     if (s->pair_nt < s->pair_split) s->pair_nt = s->pair_split;
   }
   // membrane kernel: CTAs per membrane so that small suspensions still fill the machine
@@ -981,8 +981,8 @@ extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_c
   if (pair_threads != 0 && pair_threads != 32 && pair_threads != 64 && pair_threads != 128 && pair_threads != 256)
     return fail(s, TDPD_EINVAL, "pair_threads must be 0, 32, 64, 128 or 256");
   if (list_cap != 0 && (list_cap < 4 || list_cap > 400)) return fail(s, TDPD_EINVAL, "list_cap must be 0 or 4..400");
-  if (pair_split != 0 && pair_split != 1 && pair_split != 4 && pair_split != 16)
-    return fail(s, TDPD_EINVAL, "pair_split must be 0, 1, 4 or 16");
+  if (pair_split != 0 && pair_split != 1 && pair_split != 2 && pair_split != 4 && pair_split != 16)
+    return fail(s, TDPD_EINVAL, "pair_split must be 0, 1, 2, 4 or 16");
   s->tune_nt = pair_threads;
   s->tune_split = pair_split;
   s->tune_lcap = list_cap;

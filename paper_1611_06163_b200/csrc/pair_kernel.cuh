@@ -160,10 +160,10 @@ __device__ __forceinline__ void eval_list(const DevParams& P, const PairArgs& A,
 }
 
 // RING: 1 = r_cc >= r_c (ring entries are flux-only), 2 = r_c > r_cc (ring entries are force-only)
-// SPLIT: threads per particle (1, 4 or 16; sub-wave systems): the SPLIT sub-lanes of a particle take every SPLIT-th
+// SPLIT: threads per particle (1, 2, 4 or 16; sub-wave systems): the SPLIT sub-lanes of a particle take every SPLIT-th
 // candidate of each run (adjacent addresses), keep private stacks, and their sums are combined by a fixed xor butterfly.
 template <int S, bool RANDFLUX, bool FASTW, int RING, int SPLIT>
-__global__ void __launch_bounds__(256, SPLIT == 1 ? TD_PAIR_MINB : 2) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
+__global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int NT = blockDim.x, t = threadIdx.x;
   const int lcap = A.lcap;

@@ -107,7 +107,7 @@ def test_config1_one_step_forces(T, orc):
     check_forces(sim, o, label="config1 step 3")
 
 
-@pytest.mark.parametrize("nt,cap,split", [(32, 4, 1), (64, 16, 1), (128, 0, 1), (256, 0, 1), (256, 7, 1), (128, 0, 4),
+@pytest.mark.parametrize("nt,cap,split", [(32, 4, 1), (64, 16, 1), (128, 0, 1), (256, 0, 1), (256, 7, 1), (128, 0, 2), (128, 0, 4),
                                           (64, 4, 4), (256, 0, 16), (32, 5, 16)])
 def test_pair_launch_shapes_agree(T, orc, nt, cap, split):
     # 8 x 6 x 5 cells (not powers of two: holes in the Morton rank range); tiny list caps force mid-scan flushes
