@@ -314,12 +314,20 @@ def run_ours(args) -> dict | None:
     ach = bud["flop"] / (pair_ms * 1e-3) / 1e12
     issue_peak = SM_COUNT * LANES_PER_SM * SM_MAX_MHZ * 1e6  # lane-instructions / s
     kernel_ms = {k: v["ms"] / max(K, 1) for k, v in tim.items()}
-    pair_hbm_bytes = n * (32 + 16 + 16 + 8 * max(S - 1, 0))  # pos+vel (+lo, meta) in, F4 (+Qx) out, per particle
+    # P4 + X4 + vel (+ Y2 for S > 2) in, F4 (+ Qx) out, per particle
+    pair_hbm_bytes = n * (48 + (8 if S > 2 else 0) + 16 + 4 * max(S - 1, 0))
+    traffic = None
+    try:  # measured DRAM bytes of one launch from the committed ncu capture of the same workload, if there is one
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r1_pair_traffic.json")))
+        if args.random_flux == "on" and f"config{c}" in tj:
+            traffic = tj[f"config{c}"]["dram_bytes_per_launch"]
+    except Exception:
+        pass
     roof = {
         "kernel": "k_pair", "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
         "frac": ach / FP32_PEAK_TFLOPS,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md §7); not in MEASURED_PEAKS.json",
-        "traffic": None,
+        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read + write)", "algorithmic_bytes": pair_hbm_bytes,
         "ms_per_launch": pair_ms, "flop_per_launch": bud["flop"], "share_of_step": kernel_ms["pair"] / (ms / max(K, 1)),
         "issue_slot_frac": bud["lane_instr"] / (pair_ms * 1e-3) / issue_peak,
         "hbm_gbs_algorithmic": pair_hbm_bytes / (pair_ms * 1e-3) / 1e9, "hbm_peak_gbs": hbm_peak,
