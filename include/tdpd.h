@@ -170,6 +170,14 @@ int tdpd_debug_neighbor_census(tdpd_sim* s, int32_t* n_rc, int32_t* n_rcc, uint3
 int tdpd_debug_rng(tdpd_sim* s, int64_t n, const int64_t* id_i, const int64_t* id_j, int64_t step, uint32_t tag,
                    uint32_t* words, float* gauss);
 
+/* Host-only view of the static grid tables the pair kernel uses (no CUDA device needed; for tests): ncell[3] per
+ * R-bin, cell_rank [ncells] (x-fastest linear cell -> Morton rank), and the neighbour runs of every cell in CSR form
+ * by Morton rank: seg_off [ncells + 1], seg_first [*n_runs] (first Morton rank of the run), seg_meta [*n_runs]
+ * (cells in the run | (wrap_x + 1) << 4 | (wrap_y + 1) << 6 | (wrap_z + 1) << 8).  Call once with NULL arrays to get
+ * ncell and *n_runs.  A run is a set of rank-consecutive neighbour cells of one 2x2x2 block and one periodic image. */
+int tdpd_host_grid(const tdpd_params* p, int32_t ncell[3], uint32_t* n_runs, uint32_t* cell_rank, uint32_t* seg_off,
+                   uint32_t* seg_first, uint32_t* seg_meta);
+
 /* Per-kernel timing with CUDA events on the launching streams (bench.py's roofline leg).  While enabled every
  * launch of the kernels below is bracketed by an event pair; tdpd_get_timing synchronises and returns, per
  * kernel class, the number of launches and the summed milliseconds since tdpd_set_timing(s, 1).

@@ -22,7 +22,7 @@ SYMBOLS = (
     "tdpd_create", "tdpd_load_particles", "tdpd_add_rbc_mesh", "tdpd_workspace_bytes", "tdpd_set_workspace",
     "tdpd_set_params", "tdpd_set_state", "tdpd_step", "tdpd_sync", "tdpd_get_state", "tdpd_get_forces_split",
     "tdpd_num_particles", "tdpd_num_rbc", "tdpd_get_rbc_stats", "tdpd_get_rbc_topology", "tdpd_debug_get_binning",
-    "tdpd_debug_neighbor_census", "tdpd_debug_rng", "tdpd_set_timing", "tdpd_get_timing", "tdpd_launch_count",
+    "tdpd_debug_neighbor_census", "tdpd_debug_rng", "tdpd_host_grid", "tdpd_set_timing", "tdpd_get_timing", "tdpd_launch_count",
     "tdpd_set_tuning", "tdpd_last_error", "tdpd_destroy",
 )
 
@@ -109,6 +109,7 @@ def load_library() -> C.CDLL:
     L.tdpd_debug_get_binning.argtypes = [vp, vp, vp, vp, vp]
     L.tdpd_debug_neighbor_census.argtypes = [vp, vp, vp, vp, vp]
     L.tdpd_debug_rng.argtypes = [vp, i64, vp, vp, i64, u32, vp, vp]
+    L.tdpd_host_grid.argtypes = [P(Params), vp, P(u32), vp, vp, vp, vp]
     L.tdpd_set_timing.argtypes = [vp, i32]
     L.tdpd_get_timing.argtypes = [vp, vp, vp]
     L.tdpd_launch_count.argtypes = [vp]
@@ -129,6 +130,23 @@ def _ptr(a):
 
 def _f32(a):
     return None if a is None else np.ascontiguousarray(a, dtype=np.float32)
+
+
+def host_grid(params: dict) -> dict:
+    """Static grid tables of the pair kernel (host-only; needs the built library, not a GPU)."""
+    L = load_library()
+    Pm = make_params(params)
+    nc = np.zeros(3, np.int32)
+    nr = C.c_uint32(0)
+    rc = L.tdpd_host_grid(C.byref(Pm), _ptr(nc), C.byref(nr), None, None, None, None)
+    if rc != OK:
+        raise TdpdError(rc, "tdpd_host_grid: bad parameters")
+    ncells = int(nc.prod())
+    o = dict(ncell=nc, cell_rank=np.zeros(ncells, np.uint32), seg_off=np.zeros(ncells + 1, np.uint32),
+             seg_first=np.zeros(nr.value, np.uint32), seg_meta=np.zeros(nr.value, np.uint32))
+    L.tdpd_host_grid(C.byref(Pm), _ptr(nc), C.byref(nr), _ptr(o["cell_rank"]), _ptr(o["seg_off"]), _ptr(o["seg_first"]),
+                     _ptr(o["seg_meta"]))
+    return o
 
 
 class Simulation:

@@ -944,6 +944,23 @@ extern "C" int tdpd_debug_rng(tdpd_sim* s, int64_t n, const int64_t* id_i, const
   return TDPD_OK;
 }
 
+extern "C" int tdpd_host_grid(const tdpd_params* p, int32_t ncell[3], uint32_t* n_runs, uint32_t* cell_rank,
+                              uint32_t* seg_off, uint32_t* seg_first, uint32_t* seg_meta) {
+  std::string why;
+  if (!validate_params(p, why)) return TDPD_EINVAL;
+  tdpd_sim tmp;  // host-only: no CUDA call is made
+  tmp.prm = *p;
+  derive_params(*p, tmp.dp);
+  build_grid(&tmp);
+  if (ncell) for (int a = 0; a < 3; ++a) ncell[a] = tmp.dp.ncell[a];
+  if (n_runs) *n_runs = (uint32_t)tmp.seg_first.size();
+  if (cell_rank) memcpy(cell_rank, tmp.cell_rank.data(), tmp.cell_rank.size() * 4);
+  if (seg_off) memcpy(seg_off, tmp.seg_off.data(), tmp.seg_off.size() * 4);
+  if (seg_first) memcpy(seg_first, tmp.seg_first.data(), tmp.seg_first.size() * 4);
+  if (seg_meta) memcpy(seg_meta, tmp.seg_meta.data(), tmp.seg_meta.size() * 4);
+  return TDPD_OK;
+}
+
 extern "C" int tdpd_set_timing(tdpd_sim* s, int32_t on) {
   if (!s) return TDPD_EINVAL;
   tdpd_sync(s);
