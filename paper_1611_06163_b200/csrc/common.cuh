@@ -113,6 +113,15 @@ __device__ __forceinline__ void td_box_muller(uint32_t xa, uint32_t xb, float& g
   g_sin = R * td_sin_approx(ang);
 }
 
+// cheapest variant, without the u -> 1 series: for the random-flux Gaussians of ring entries, whose amplitude
+// m_s sqrt(kappa rho C / dt) is ~1e-2 of the Fickian flux, so the 5e-5 absolute error of lg2.approx near u = 1 is nil
+__device__ __forceinline__ void td_box_muller_fast(uint32_t xa, uint32_t xb, float& g_cos, float& g_sin) {
+  const float R = td_sqrt_approx(-1.3862943611198906f * td_lg2_approx(td_uniform(xa)));
+  const float ang = 6.283185307179586f * td_uniform(xb);
+  g_cos = R * td_cos_approx(ang);
+  g_sin = R * td_sin_approx(ang);
+}
+
 // full-precision variant (libdevice logf / sincospif, ~1 ulp) for the membrane kernel: bond random forces carry the
 // prefactor sqrt(2 kBT/dt) sqrt(2 gamma_T) ~ 35, so the 1e-5 absolute error of the MUFU path would cost 1e-3 in the
 // force of a vertex; there are only ~4 bonds per membrane vertex, so the cost is nil

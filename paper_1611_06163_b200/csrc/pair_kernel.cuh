@@ -87,11 +87,12 @@ __device__ __forceinline__ void pair_eval(const DevParams& P, const PairArgs& A,
     const uint32_t lo = min(me.id, idj), hi = max(me.id, idj);
     uint32_t x0, x1, x2, x3;
     td_philox(lo, hi, A.step, 0u, P.key0, P.key1, x0, x1, x2, x3);
-    td_box_muller(x0, x1, g0, g1);
-    if (FLUX && RANDFLUX && S >= 2) td_box_muller(x2, x3, g2, g3);
+    if (FORCE) td_box_muller(x0, x1, g0, g1);  // g0 = xi of the random force
+    else td_box_muller_fast(x0, x1, g0, g1);    // flux-only entry: zeta alone
+    if (FLUX && RANDFLUX && S >= 2) td_box_muller_fast(x2, x3, g2, g3);
     if (FLUX && RANDFLUX && S >= 3) {
       td_philox(lo, hi, A.step, 4u, P.key0, P.key1, x0, x1, x2, x3);
-      td_box_muller(x0, x1, g4, g5);
+      td_box_muller_fast(x0, x1, g4, g5);
     }
   }
   if (FLUX) {
