@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ hist,
     if (i0 + k < total) hist[i0 + k] = excl;
     excl += v[k];
   }
-  if (threadIdx.x == 0) tops[blockIdx.x] = sum;
+  if (threadIdx.x == 0) tops[blockIdx.x] = gridDim.x == 1 ? 0u : sum;  // a single chunk needs no second level
 }
 
 __global__ void __launch_bounds__(1024) k_sort_scan_tops(uint32_t* __restrict__ tops, int nchunk) {
@@ -204,11 +204,11 @@ int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits
     int shift = p * RB;
     k_sort_hist<<<nblk, SORT_NT, 0, st>>>(keys[side], n, shift, hist, nblk);
     k_sort_scan<<<nchunk, 1024, 0, st>>>(hist, nh, tops);
-    k_sort_scan_tops<<<1, 1024, 0, st>>>(tops, nchunk);
+    if (nchunk > 1) k_sort_scan_tops<<<1, 1024, 0, st>>>(tops, nchunk);
     k_sort_scatter<<<nblk, SORT_NT, 0, st>>>(keys[side], vals[side], keys[side ^ 1], vals[side ^ 1], n, shift, hist,
                                               nblk, tops);
     side ^= 1;
-    if (n_launches) *n_launches += 4;
+    if (n_launches) *n_launches += nchunk > 1 ? 4 : 3;
   }
   return side;
 }
