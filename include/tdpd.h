@@ -195,6 +195,10 @@ int64_t tdpd_launch_count(const tdpd_sim* s);
  * {1, 2, 4, 16} = threads per particle (sub-wave systems); 0 = automatic.  ESTATE after tdpd_set_workspace. */
 int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap, int32_t pair_split);
 
+/* Steps are replayed as CUDA graphs (one per ping-pong side x first/last step of a call, captured on first use) unless
+ * per-kernel timing is on; on = 0 switches to plain launches.  Results are bit-identical either way. */
+int tdpd_set_graph(tdpd_sim* s, int32_t on);
+
 const char* tdpd_last_error(const tdpd_sim* s);
 int tdpd_destroy(tdpd_sim* s);
 

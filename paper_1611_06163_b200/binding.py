@@ -23,7 +23,7 @@ SYMBOLS = (
     "tdpd_set_params", "tdpd_set_state", "tdpd_step", "tdpd_sync", "tdpd_get_state", "tdpd_get_forces_split",
     "tdpd_num_particles", "tdpd_num_rbc", "tdpd_get_rbc_stats", "tdpd_get_rbc_topology", "tdpd_debug_get_binning",
     "tdpd_debug_neighbor_census", "tdpd_debug_rng", "tdpd_host_grid", "tdpd_set_timing", "tdpd_get_timing", "tdpd_launch_count",
-    "tdpd_set_tuning", "tdpd_last_error", "tdpd_destroy",
+    "tdpd_set_tuning", "tdpd_set_graph", "tdpd_last_error", "tdpd_destroy",
 )
 
 
@@ -115,6 +115,7 @@ def load_library() -> C.CDLL:
     L.tdpd_launch_count.argtypes = [vp]
     L.tdpd_launch_count.restype = i64
     L.tdpd_set_tuning.argtypes = [vp, i32, i32, i32]
+    L.tdpd_set_graph.argtypes = [vp, i32]
     L.tdpd_last_error.argtypes = [vp]
     L.tdpd_last_error.restype = C.c_char_p
     L.tdpd_destroy.argtypes = [vp]
@@ -314,6 +315,9 @@ class Simulation:
         g = np.zeros((len(id_i), 4), np.float32)
         self._ck(self.L.tdpd_debug_rng(self.h, len(id_i), _ptr(id_i), _ptr(id_j), step, tag, _ptr(w), _ptr(g)))
         return w, g
+
+    def set_graph(self, on: bool):
+        self._ck(self.L.tdpd_set_graph(self.h, int(on)))
 
     def set_timing(self, on: bool):
         self._ck(self.L.tdpd_set_timing(self.h, int(on)))

@@ -72,6 +72,7 @@ struct tdpd_sim {
   float4 *F4 = nullptr, *Fb = nullptr;
   float *Qx = nullptr, *staging = nullptr;
   int* err_d = nullptr;
+  uint32_t* step_d = nullptr;  // device copy of the step word (the integrator bumps it)
   double* stats_d = nullptr;
   RbcDev* rbcs_d = nullptr;
   MeshTemplateDev* tmpls_d = nullptr;
@@ -80,6 +81,11 @@ struct tdpd_sim {
   int64_t n = 0, step = 0;
   bool have_forces = false, binned = false;
   bool timing = false;
+  // CUDA graphs of one step, by [side of the ping-pong][first step of a call][last step of a call]
+  bool use_graph = true;
+  cudaGraphExec_t gexec[2][2][2] = {};
+  int glaunches[2][2][2] = {};
+  uint32_t* gkeys[2][2][2] = {};
   Timer timers[TDPD_N_TIMERS];
   int64_t launches = 0;
   std::string err;
@@ -491,6 +497,7 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->Qx = c.take<float>(n * (size_t)std::max(S - 1, 1));
   s->staging = c.take<float>(n * 4 * 3);  // up to three id-ordered arrays of <= 4 floats per particle
   s->err_d = c.take<int>(64);
+  s->step_d = c.take<uint32_t>(64);
   size_t M = s->rbcs.size();
   s->stats_d = c.take<double>(2 * std::max<size_t>(M, 1));
   s->rbcs_d = c.take<RbcDev>(std::max<size_t>(M, 1));
@@ -643,7 +650,7 @@ int bin_and_sort(tdpd_sim* s, int mode /*0 keys only, 1 open, 2 close+open*/) {
     Scope t(s, 0, s->sA);
     if (mode == 0) td_launch_init_keys(s->dp, s->st[c], s->n, s->keys[0], s->vals[0], s->cell_rank_d, s->sA);
     else td_launch_kick_drift_key(s->dp, s->st[c], s->F4, s->Qx, s->Fb, s->n, s->keys[0], s->vals[0], s->cell_rank_d,
-                                  mode == 2, s->sA);
+                                  mode == 2, s->step_d, s->sA);
     s->launches += 1; s->timers[0].launches += 1;
   }
   int side, nl = 0;
@@ -678,7 +685,7 @@ int eval_forces(tdpd_sim* s) {
     A.rec = s->rec; A.vel = s->st[c].vel; A.pos = s->st[c].pos; A.lo = s->st[c].lo; A.keys = s->keys_sorted;
     A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
     A.seg_off = s->seg_off_d; A.seg_first = s->seg_first_d; A.seg_meta = s->seg_meta_d;
-    A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step = (uint32_t)s->step; A.lcap = s->lcap; A.err = s->err_d;
+    A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step_p = s->step_d; A.lcap = s->lcap; A.err = s->err_d;
     int rc = td_launch_pair(s->dp, A, s->pair_nt, s->pair_split, s->sA);
     if (rc) return fail(s, TDPD_ECUDA, std::string("pair kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
     s->launches += 1; s->timers[3].launches += 1;
@@ -689,7 +696,7 @@ int eval_forces(tdpd_sim* s) {
       MembraneArgs M;
       M.st = s->st[c]; M.slot_of_id = s->slot_of_id; M.rbcs = s->rbcs_d; M.tmpls = s->tmpls_d;
       M.h0 = s->h0_d; M.kp = s->kp_d; M.A0t = s->A0t_d; M.Fb = s->Fb; M.stats = s->stats_d;
-      M.nchunk = s->mem_nchunk; M.step = (uint32_t)s->step; M.err = s->err_d;
+      M.nchunk = s->mem_nchunk; M.step_p = s->step_d; M.err = s->err_d;
       int rc = td_launch_membrane(s->dp, M, (int)s->rbcs.size(), s->max_nv, s->mem_nt, s->sB);
       if (rc) return fail(s, TDPD_ECUDA, std::string("membrane kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
       s->launches += 1; s->timers[4].launches += 1;
@@ -712,25 +719,74 @@ int ensure_forces(tdpd_sim* s) {
 }
 }  // namespace
 
+namespace {
+// enqueues one velocity-Verlet step: opening half-kick (fused with the closing one of the previous step of this call),
+// drift, binning, forces, and the closing half-kick if this is the last step of the call
+int enqueue_step(tdpd_sim* s, bool first, bool last) {
+  int rc = bin_and_sort(s, first ? 1 : 2);
+  if (rc) return rc;
+  rc = eval_forces(s);
+  if (rc) return rc;
+  if (last) {
+    Scope t(s, 5, s->sA);
+    td_launch_kick(s->dp, s->st[s->cur], s->F4, s->Qx, s->Fb, s->n, s->sA);
+    s->launches += 1; s->timers[5].launches += 1;
+  }
+  CK(cudaGetLastError());
+  return TDPD_OK;
+}
+
+void drop_graphs(tdpd_sim* s) {
+  for (auto& a : s->gexec) for (auto& b : a) for (auto& g : b) { if (g) cudaGraphExecDestroy(g); g = nullptr; }
+}
+}  // namespace
+
 extern "C" int tdpd_step(tdpd_sim* s, int32_t nsteps) {
   if (!s) return TDPD_EINVAL;
   if (nsteps < 0) return fail(s, TDPD_EINVAL, "nsteps < 0");
   int rc = ensure_forces(s);
   if (rc || nsteps == 0) return rc;
   for (int32_t it = 0; it < nsteps; ++it) {
-    // opening half-kick + drift + wrap + key (fused with the closing half-kick of the previous step of this call)
-    rc = bin_and_sort(s, it == 0 ? 1 : 2);
-    if (rc) return rc;
-    s->step += 1;
-    rc = eval_forces(s);
-    if (rc) return rc;
+    const bool first = it == 0, last = it == nsteps - 1;
+    s->step += 1;  // the integrator bumps the device copy
+    if (!s->use_graph || s->timing || s->n == 0) {
+      if ((rc = enqueue_step(s, first, last))) return rc;
+      continue;
+    }
+    // one CUDA graph per (ping-pong side, first, last): the launch sequence of a step is static, and the step word
+    // lives in device memory, so replaying the graph is all a step needs
+    const int side = s->cur;
+    cudaGraphExec_t& ge = s->gexec[side][first][last];
+    if (!ge) {
+      const int64_t l0 = s->launches;
+      cudaGraph_t g = nullptr;
+      bool ok = cudaStreamBeginCapture(s->sA, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+      if (ok) {
+        rc = enqueue_step(s, first, last);
+        ok = cudaStreamEndCapture(s->sA, &g) == cudaSuccess && rc == TDPD_OK && g;
+        ok = ok && cudaGraphInstantiate(&ge, g, 0) == cudaSuccess;
+        if (g) cudaGraphDestroy(g);
+      }
+      if (!ok) {  // capture is not available here: fall back to plain launches for good
+        cudaGetLastError();
+        ge = nullptr;
+        s->use_graph = false;
+        drop_graphs(s);
+        s->cur = side;
+        if ((rc = enqueue_step(s, first, last))) return rc;
+        continue;
+      }
+      s->glaunches[side][first][last] = (int)(s->launches - l0);
+      s->gkeys[side][first][last] = s->keys_sorted;
+      s->launches = l0;  // counted at launch below
+      s->cur = side;     // the capture advanced the host bookkeeping; the launch below does it again
+    }
+    CK(cudaGraphLaunch(ge, s->sA));
+    s->cur = side ^ 1;
+    s->keys_sorted = s->gkeys[side][first][last];
+    s->launches += s->glaunches[side][first][last];
+    s->binned = true; s->have_forces = true;
   }
-  {
-    Scope t(s, 5, s->sA);
-    td_launch_kick(s->dp, s->st[s->cur], s->F4, s->Qx, s->Fb, s->n, s->sA);
-    s->launches += 1; s->timers[5].launches += 1;
-  }
-  CK(cudaGetLastError());
   return TDPD_OK;
 }
 
@@ -852,6 +908,7 @@ extern "C" int tdpd_set_params(tdpd_sim* s, const tdpd_params* p) {
   s->prm = *p;
   s->dp = d;
   s->have_forces = false;
+  drop_graphs(s);  // the parameters are baked into the captured kernel nodes
   return TDPD_OK;
 }
 
@@ -1006,6 +1063,13 @@ extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_c
   return TDPD_OK;
 }
 
+extern "C" int tdpd_set_graph(tdpd_sim* s, int32_t on) {
+  if (!s) return TDPD_EINVAL;
+  s->use_graph = on != 0;
+  if (!on) drop_graphs(s);
+  return TDPD_OK;
+}
+
 extern "C" const char* tdpd_last_error(const tdpd_sim* s) { return s ? s->err.c_str() : "null handle"; }
 
 extern "C" int tdpd_destroy(tdpd_sim* s) {
@@ -1015,6 +1079,7 @@ extern "C" int tdpd_destroy(tdpd_sim* s) {
   cudaStreamSynchronize(s->sB);
   for (auto& t : s->timers)
     for (auto& e : t.ev) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
+  drop_graphs(s);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->own_streams) { cudaStreamDestroy(s->sA); cudaStreamDestroy(s->sB); }

@@ -168,7 +168,7 @@ struct PairArgs {
   float4* F4;                  // Fx, Fy, Fz, Q_0 by slot
   float* Qx;                   // [(S-1)][n]
   int64_t n;
-  uint32_t step;               // RNG step word
+  const uint32_t* step_p;      // RNG step word (device counter, bumped by the integrator: lets a step be a CUDA graph)
   int lcap;                    // list entries per thread
   int* err;                    // device error word
 };
@@ -206,7 +206,7 @@ struct MembraneArgs {
   float4* Fb;       // bonded force by id
   double* stats;    // [M][2] area, volume
   int nchunk;       // CTAs per membrane
-  uint32_t step;
+  const uint32_t* step_p;  // RNG step word (device counter)
   int* err;
 };
 
@@ -221,7 +221,7 @@ void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, ui
                          const uint32_t* cell_rank, cudaStream_t st);
 void td_launch_kick_drift_key(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
                               const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
-                              bool closing_first, cudaStream_t st);
+                              bool closing_first, uint32_t* step_d, cudaStream_t st);
 void td_launch_kick(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx, const float4* Fb,
                     int64_t n, cudaStream_t st);
 int td_sort_passes(int key_bits);

@@ -71,9 +71,11 @@ template <int S>
 __global__ void __launch_bounds__(256) k_integrate(const DevParams P, SortedState st, const float4* __restrict__ F4,
                                                    const float* __restrict__ Qx, const float4* __restrict__ Fb,
                                                    int64_t n, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
-                                                   const uint32_t* __restrict__ cell_rank, int mode) {
+                                                   const uint32_t* __restrict__ cell_rank, int mode,
+                                                   uint32_t* __restrict__ step_d) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  if (i == 0 && step_d) *step_d += 1u;  // the force evaluation that follows the drift uses the next step word
   float4 p = st.pos[i];
   if (mode != 0) {
     float4 v = st.vel[i];
@@ -103,27 +105,27 @@ __global__ void __launch_bounds__(256) k_integrate(const DevParams P, SortedStat
 
 static void launch_integrate(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
                              const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
-                             int mode, cudaStream_t st) {
+                             int mode, uint32_t* step_d, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
   switch (P.n_species) {
-    case 1: k_integrate<1><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
-    case 2: k_integrate<2><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
-    case 3: k_integrate<3><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
-    default: k_integrate<4><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode); break;
+    case 1: k_integrate<1><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
+    case 2: k_integrate<2><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
+    case 3: k_integrate<3><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
+    default: k_integrate<4><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
   }
 }
 
 void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
                          const uint32_t* cell_rank, cudaStream_t st) {
-  launch_integrate(P, s, nullptr, nullptr, nullptr, n, keys, vals, cell_rank, 0, st);
+  launch_integrate(P, s, nullptr, nullptr, nullptr, n, keys, vals, cell_rank, 0, nullptr, st);
 }
 void td_launch_kick_drift_key(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
                               const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
-                              bool closing_first, cudaStream_t st) {
-  launch_integrate(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, closing_first ? 2 : 1, st);
+                              bool closing_first, uint32_t* step_d, cudaStream_t st) {
+  launch_integrate(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, closing_first ? 2 : 1, step_d, st);
 }
 void td_launch_kick(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx, const float4* Fb,
                     int64_t n, cudaStream_t st) {
-  launch_integrate(P, s, F4, Qx, Fb, n, nullptr, nullptr, nullptr, 3, st);
+  launch_integrate(P, s, F4, Qx, Fb, n, nullptr, nullptr, nullptr, 3, nullptr, st);
 }

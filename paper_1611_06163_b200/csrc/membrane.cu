@@ -36,6 +36,7 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[2][8];
   __shared__ double tot[2];
+  const uint32_t step = __ldg(A.step_p);
   const int m = blockIdx.x / A.nchunk, chunk = blockIdx.x % A.nchunk;
   const RbcDev R = A.rbcs[m];
   const MeshTemplateDev T = A.tmpls[R.tmpl];
@@ -115,7 +116,7 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
       for (int row = 0; row < 3; ++row) {
         uint32_t x0, x1, x2, x3;
         float g0, g1, g2, g3;
-        td_philox(lo, hi, A.step, 1u + row, P.key0, P.key1, x0, x1, x2, x3);
+        td_philox(lo, hi, step, 1u + row, P.key0, P.key1, x0, x1, x2, x3);
         td_box_muller_precise(x0, x1, g0, g1);
         td_box_muller_precise(x2, x3, g2, g3);
         N[3 * row] = g0; N[3 * row + 1] = g1; N[3 * row + 2] = g2;

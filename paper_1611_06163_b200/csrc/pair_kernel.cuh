@@ -60,7 +60,7 @@ struct Self {  // the thread's own particle
   float x, y, z;
   float4 v;  // vx, vy, vz, C_0
   float c[TD_S];
-  uint32_t id, meta;
+  uint32_t id, meta, step;
   int lc27;  // 27 * local cell index
 };
 
@@ -86,12 +86,12 @@ __device__ __forceinline__ void pair_eval(const DevParams& P, const PairArgs& A,
   if (FORCE || RANDFLUX) {
     const uint32_t lo = min(me.id, idj), hi = max(me.id, idj);
     uint32_t x0, x1, x2, x3;
-    td_philox(lo, hi, A.step, 0u, P.key0, P.key1, x0, x1, x2, x3);
+    td_philox(lo, hi, me.step, 0u, P.key0, P.key1, x0, x1, x2, x3);
     if (FORCE) td_box_muller(x0, x1, g0, g1);  // g0 = xi of the random force
     else td_box_muller_fast(x0, x1, g0, g1);    // flux-only entry: zeta alone
     if (FLUX && RANDFLUX && S >= 2) td_box_muller_fast(x2, x3, g2, g3);
     if (FLUX && RANDFLUX && S >= 3) {
-      td_philox(lo, hi, A.step, 4u, P.key0, P.key1, x0, x1, x2, x3);
+      td_philox(lo, hi, me.step, 4u, P.key0, P.key1, x0, x1, x2, x3);
       td_box_muller_fast(x0, x1, g4, g5);
     }
   }
@@ -195,6 +195,7 @@ __global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constan
     me.c[0] = x.x; me.c[1] = x.y; me.c[2] = 0.f; me.c[3] = 0.f;
     if (S > 2) { const float2 y = __ldg(&A.rec.Y2[is]); me.c[2] = y.x; me.c[3] = y.y; }
     me.lc27 = 0;
+    me.step = __ldg(A.step_p);
   }
   // ---- type-pair tables
   for (int k = t; k < 16; k += NT) {

@@ -220,6 +220,21 @@ def test_step_batching_and_determinism(T):
         assert np.array_equal(ga[k], gc[k]), k
 
 
+def test_cuda_graph_replay_is_bit_identical(T):
+    w = W.small_suspension(seed=4, box=(18, 18, 8), n_rbc=1, n_species=2)
+    a = T.Simulation.from_workload(w)            # steps replayed as CUDA graphs (default)
+    b = T.Simulation.from_workload(w)
+    b.set_graph(False)                           # plain launches
+    for k in (1, 3, 1, 6):                       # first / middle / last steps of a call, both ping-pong sides
+        a.step(k)
+        b.step(k)
+    ga, gb = a.get_state(), b.get_state()
+    assert ga["step"] == gb["step"] == 11
+    for k in ("pos", "vel", "conc", "force", "flux"):
+        assert np.array_equal(ga[k], gb[k]), k
+    assert a.launch_count == b.launch_count
+
+
 def test_pair_momentum_and_flux_sums(T):
     w = W.config(3)
     sim = T.Simulation.from_workload(w)
