@@ -275,6 +275,7 @@ def run_ours(args) -> dict | None:
         return t, nl
 
     # ---- device-timed region: K steps as a user runs them (steps replayed as CUDA graphs)
+    timed_steps()  # untimed pass with the same call pattern: every CUDA graph the timed pass replays is captured here
     clocks = ClockSampler(local) if rank == 0 else None
     ms, launches = timed_steps()
     # ---- the same K steps again with per-kernel-class CUDA events on the launching streams (plain launches: the
@@ -344,7 +345,7 @@ def run_ours(args) -> dict | None:
     }
     out = {
         "metric": "tDPD particle-steps/sec", "value": ntot * K / (tmax * 1e-3), "unit": "particle-steps/s",
-        "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": tmax / K, "higher_is_better": True,
+        "n_gpus": world, "steps": K, "warmup": Wm + K, "ms_per_step": tmax / K, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config{c}", "n_particles": n, "n_rbc": sim.n_rbc, "n_species": S,
                    "box": [float(x) for x in w.params["box"]], "random_flux": bool(np.any(w.params["m_s"][:S] != 0)),
