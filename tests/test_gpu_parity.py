@@ -367,3 +367,41 @@ def test_pairs_at_the_force_cutoff(T, orc):
             assert np.all(g["force"][k] == 0) and np.all(r["force"][k] == 0)
         else:
             assert np.any(r["force"][k] != 0) and np.any(g["force"][k] != 0)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# BASELINE.json's full run lengths (100 / 1000 / 1000 / 500 / 200 steps): the invariants that hold at any size
+@pytest.mark.parametrize("c", [1, 2, 3, 4, 5])
+def test_full_length_run_invariants(T, c):
+    w = W.config(c)
+    sim = T.Simulation.from_workload(w)
+    g0 = sim.get_state(forces=False)
+    sim.step(w.steps)
+    g = sim.get_state()                              # raises TdpdError (EUNSTABLE) on NaN / overstretched bonds
+    assert g["step"] == w.steps
+    n, S = len(g["pos"]), g["conc"].shape[1]
+    box = np.asarray(w.params["box"], np.float64)
+    assert np.all(g["pos"] >= 0) and np.all(g["pos"] < box.astype(np.float32))
+    # total concentration of every species is conserved (no sources; the random flux is antisymmetric)
+    for s in range(S):
+        c0, c1 = g0["conc"][:, s].astype(np.float64).sum(), g["conc"][:, s].astype(np.float64).sum()
+        assert abs(c1 - c0) <= 1e-4 * max(abs(c0), 1.0), (s, c0, c1)
+    # momentum: pair and bonded forces sum to zero; the double-Poiseuille body force adds +f and -f on the two halves,
+    # so the net momentum per particle stays far below the thermal velocity
+    v = g["vel"].astype(np.float64)
+    assert np.abs(v.mean(axis=0)).max() < 2e-2
+    # kinetic temperature of the solvent stays at k_BT (dt = 0.01 integration error and the driven flow add < 5 %)
+    ns = w.n_solvent
+    vs = v[:ns] - v[:ns].mean(axis=0)
+    if w.rbcs:   # remove the driven flow profile u_x(z) before measuring the temperature
+        zb = np.minimum((g["pos"][:ns, 2] / box[2] * 32).astype(int), 31)
+        ux = np.bincount(zb, weights=vs[:, 0], minlength=32) / np.maximum(np.bincount(zb, minlength=32), 1)
+        vs[:, 0] -= ux[zb]
+    kT = (vs ** 2).sum() / (3 * ns - 3)
+    assert abs(kT - 1.0) < 0.05, kT
+    if w.rbcs:   # membranes hold area and volume near their targets: 0.5 % for a cell (the oracle's pin on config 3),
+        st = sim.rbc_stats()                        # 1 % for the worst of the 1000 cells of config 5
+        da, dv = np.abs(st["area"] / st["A0"] - 1), np.abs(st["volume"] / st["V0"] - 1)
+        print(f"[invariants] config{c}: kT = {kT:.4f}, max |dA/A0| = {da.max():.2e}, max |dV/V0| = {dv.max():.2e}")
+        assert np.median(da) < 5e-3 and np.median(dv) < 5e-3
+        assert da.max() < (5e-3 if len(da) <= 100 else 1e-2) and dv.max() < (5e-3 if len(dv) <= 100 else 1e-2)
