@@ -405,3 +405,46 @@ def test_full_length_run_invariants(T, c):
         print(f"[invariants] config{c}: kT = {kT:.4f}, max |dA/A0| = {da.max():.2e}, max |dV/V0| = {dv.max():.2e}")
         assert np.median(da) < 5e-3 and np.median(dv) < 5e-3
         assert da.max() < (5e-3 if len(da) <= 100 else 1e-2) and dv.max() < (5e-3 if len(dv) <= 100 else 1e-2)
+
+
+def test_config2_concentration_step_relaxes_with_tdpd_diffusivity(T):
+    """BASELINE config 2 at full size and length: the x < 16 concentration step of the periodic 32^3 box is a square
+    wave whose mode k decays as exp(-D k^2 t) with D = D^F + D^zeta (Eq 11-12) evaluated with the
+    run's own g(r) — the same closed forms the oracle is pinned to in tests/test_oracle_dynamics.py."""
+    from scipy.spatial import cKDTree
+
+    w = W.config(2)
+    L = float(w.params["box"][0])
+    sim = T.Simulation.from_workload(w)
+    sim.step(100)                                             # let g(r) equilibrate
+    k1 = 2 * np.pi / L
+    ts, amp = [], []
+    for _ in range(46):
+        s = sim.get_state(forces=False)
+        amp.append(2 * np.mean(s["conc"][:, 0].astype(np.float64) * np.sin(k1 * s["pos"][:, 0].astype(np.float64))))
+        ts.append(s["step"] * 0.01)
+        sim.step(20)
+    rate = -np.polyfit(ts, np.log(amp), 1)[0]
+    D_meas = rate / k1 ** 2
+    x = np.mod(sim.get_state(forces=False)["pos"].astype(np.float64), L)
+    tree = cKDTree(x, boxsize=L)
+    sub = cKDTree(x[::16], boxsize=L)
+    edges = np.linspace(0, 1.58, 80)
+    cum = sub.count_neighbors(tree, edges).astype(np.float64)
+    hist = np.diff(cum)
+    rm = 0.5 * (edges[1:] + edges[:-1]); dr = edges[1] - edges[0]
+    rho = len(x) / L ** 3
+    g = hist / (sub.n * rho * 4 * np.pi * rm ** 2 * dr)
+    kappa, gamma, kBT, rcc = 10.0, 4.5, 1.0, 1.58
+    DF = 2 * np.pi * kappa * rho / 3 * np.sum(rm ** 4 * (1 - rm / rcc) ** 2 * g) * dr
+    Dz = 3 * kBT / (4 * np.pi * gamma * rho * np.sum(rm ** 2 * np.clip(1 - rm, 0, None) * g) * dr)
+    print(f"[diffusion] config2: D measured {D_meas:.3f}, D^F + D^zeta = {DF:.3f} + {Dz:.3f}")
+    assert D_meas == pytest.approx(DF + Dz, rel=0.06)
+    # the profile itself after t = 10.2: odd modes of the square wave, C(x) = 1/2 + sum 2/(k pi) sin(k k1 x) e^{-D k^2 k1^2 t}
+    s = sim.get_state(forces=False)
+    t_end = s["step"] * 0.01
+    xb = (np.arange(32) + 0.5) * L / 32
+    ib = np.minimum((s["pos"][:, 0] / L * 32).astype(int), 31)
+    prof = np.bincount(ib, weights=s["conc"][:, 0], minlength=32) / np.bincount(ib, minlength=32)
+    ref = 0.5 + sum(2 / (k * np.pi) * np.sin(k * k1 * xb) * np.exp(-(DF + Dz) * (k * k1) ** 2 * t_end) for k in (1, 3, 5))
+    assert np.abs(prof - ref).max() < 0.02
