@@ -448,3 +448,54 @@ def test_config2_concentration_step_relaxes_with_tdpd_diffusivity(T):
     prof = np.bincount(ib, weights=s["conc"][:, 0], minlength=32) / np.bincount(ib, minlength=32)
     ref = 0.5 + sum(2 / (k * np.pi) * np.sin(k * k1 * xb) * np.exp(-(DF + Dz) * (k * k1) ** 2 * t_end) for k in (1, 3, 5))
     assert np.abs(prof - ref).max() < 0.02
+
+
+def test_transient_double_poiseuille_flow(T):
+    """SURVEY §8(f) row 4 / PAPER.md:178-184 (Fig 5): 256,000 particles in a periodic 40^3 box, alpha = 18.75,
+    gamma = 4.5, r_c = 1.58, s = 0.41, body force +f for z < d and -f for z > d (d = 20).  The velocity profile must
+    follow the analytic transient of the diffusion equation u_t = nu u_zz + g(z) started from rest,
+        u(z, t) = sum_{n odd} 4 f / (n pi nu k_n^2) (1 - exp(-nu k_n^2 t)) sin(k_n z),   k_n = n pi / d,
+    at the paper's snapshot times t = 3, 6, 12, 24 with the ONE viscosity fitted to the steady profile at t = 48."""
+    f, d, L = 0.05, 20.0, 40.0
+    w = W.make_fluid("poiseuille", (L, L, L), 4.0, seed=W.BASE_SEED + 11, conc="zero", a=18.75, gamma=4.5, s_R=0.41,
+                     r_c=1.58, r_cc=1.58, m_s=0.0, body=f, body_mode=W.BODY_DOUBLE_POISEUILLE_Z)
+    assert w.n_total == 256000
+    sim = T.Simulation.from_workload(w)
+    nb = 40
+    zc = (np.arange(nb) + 0.5) * L / nb
+
+    def profile(nsamp=25, every=4):          # u_x(z) averaged over nsamp snapshots (100 steps = 1 time unit)
+        acc = np.zeros(nb)
+        for _ in range(nsamp):
+            s = sim.get_state(forces=False)
+            ib = np.minimum((s["pos"][:, 2] / L * nb).astype(int), nb - 1)
+            acc += np.bincount(ib, weights=s["vel"][:, 0], minlength=nb) / np.bincount(ib, minlength=nb)
+            sim.step(every)
+        return acc / nsamp
+
+    snaps, t_now = {}, 0.0
+    for t_snap in (3.0, 6.0, 12.0, 24.0, 48.0):
+        sim.step(int(round((t_snap - 0.5 - t_now) * 100)))
+        snaps[t_snap] = profile()            # centred on t_snap: covers [t_snap - 0.5, t_snap + 0.5]
+        t_now = t_snap + 0.5
+
+    def series(nu, t):
+        u = np.zeros(nb)
+        for n in range(1, 60, 2):
+            k = n * np.pi / d
+            u += 4 * f / (n * np.pi * nu * k * k) * (1 - np.exp(-nu * k * k * t)) * np.sin(k * zc)
+        return u
+
+    # one-parameter fit of nu to the t = 48 profile (the series is linear in 1/nu up to the small transient rest)
+    nus = np.linspace(0.5, 30.0, 1200)
+    err = [np.abs(series(nu, 48.0) - snaps[48.0]).max() for nu in nus]
+    nu = float(nus[int(np.argmin(err))])
+    umax = np.abs(series(nu, 48.0)).max()
+    print(f"[poiseuille] nu = {nu:.3f} (eta = {4 * nu:.2f}), u_max = {umax:.4f}, residual at t = 48: {min(err) / umax:.3f}")
+    assert min(err) < 0.04 * umax                          # parabolic in both halves, antisymmetric
+    for t_snap in (3.0, 6.0, 12.0, 24.0):
+        dev = np.abs(series(nu, t_snap) - snaps[t_snap]).max()
+        print(f"[poiseuille] t = {t_snap}: max deviation / u_max = {dev / umax:.3f}")
+        assert dev < 0.06 * umax, (t_snap, dev / umax)
+    vy = sim.get_state(forces=False)["vel"][:, 1]
+    assert abs(vy.mean()) < 5e-3                            # no flow across the force
