@@ -418,12 +418,18 @@ def test_config2_concentration_step_relaxes_with_tdpd_diffusivity(T):
     sim = T.Simulation.from_workload(w)
     sim.step(100)                                             # let g(r) equilibrate
     k1 = 2 * np.pi / L
-    ts, amp = [], []
+    ts, amp, kTs = [], [], []
     for _ in range(46):
         s = sim.get_state(forces=False)
         amp.append(2 * np.mean(s["conc"][:, 0].astype(np.float64) * np.sin(k1 * s["pos"][:, 0].astype(np.float64))))
         ts.append(s["step"] * 0.01)
+        v = s["vel"].astype(np.float64)
+        v -= v.mean(axis=0)
+        kTs.append((v ** 2).sum() / (3 * len(v) - 3))
         sim.step(20)
+    # equilibrium temperature (BASELINE north_star: k_BT within 1 %), time-averaged over steps 100..1000
+    print(f"[temperature] config2: <kT> = {np.mean(kTs):.4f} +- {np.std(kTs):.4f}")
+    assert abs(np.mean(kTs) - 1.0) < 0.01
     rate = -np.polyfit(ts, np.log(amp), 1)[0]
     D_meas = rate / k1 ** 2
     x = np.mod(sim.get_state(forces=False)["pos"].astype(np.float64), L)
