@@ -505,3 +505,52 @@ def test_transient_double_poiseuille_flow(T):
         assert dev < 0.06 * umax, (t_snap, dev / umax)
     vy = sim.get_state(forces=False)["vel"][:, 1]
     assert abs(vy.mean()) < 5e-3                            # no flow across the force
+
+
+def test_error_paths_of_the_boundary(T):
+    """include/tdpd.h: every misuse returns its error code (raised as TdpdError by the binding), nothing aborts."""
+    import ctypes as C
+    p = W.fluid_params((20, 20, 20), 3.0, seed=5, n_types=3)
+    pos = np.array([[1, 1, 1], [2, 2, 2]], np.float32)
+
+    def code(fn):
+        with pytest.raises(T.TdpdError) as e:
+            fn()
+        return e.value.code
+
+    s = T.Simulation(p)
+    assert code(lambda: s.load_particles(pos, None, np.array([0, 3], np.int32))) == -1       # type out of range
+    s.load_particles(pos)
+    rp = dict(W.rbc_params(), gamma_T=np.float32(7.0), gamma_C=np.float32(2.0))             # 3 gamma_C < gamma_T
+    from tdpd_workloads import mesh as M
+    verts, tris = M.rbc_mesh(1)
+    v = (verts + 10.0).astype(np.float32)
+    small = T.Simulation(W.fluid_params((8, 8, 8), 3.0, seed=5, n_types=3))
+    assert code(lambda: small.add_rbc_mesh((verts + 4.0).astype(np.float32), None, None, tris, W.rbc_params())) == -1  # > box/2
+    assert code(lambda: s.add_rbc_mesh(v, None, None, tris, rp)) == -1
+    assert code(lambda: s.add_rbc_mesh(v, None, None, tris[:, ::-1][:-1], W.rbc_params())) == -1   # not closed
+    k = s.add_rbc_mesh(v, None, None, tris, W.rbc_params())
+    assert k == 0 and s.n == 2 + len(v)
+    # workspace too small / unaligned
+    need = C.c_size_t(0)
+    assert s.L.tdpd_workspace_bytes(s.h, C.byref(need)) == 0 and need.value > 0
+    import torch
+    buf = torch.empty(need.value + 512, dtype=torch.uint8, device="cuda:0")
+    base = (buf.data_ptr() + 255) & ~255
+    assert s.L.tdpd_set_workspace(s.h, C.c_void_p(base), C.c_size_t(need.value - 1)) == -3   # ENOMEM
+    assert s.L.tdpd_set_workspace(s.h, C.c_void_p(base + 8), need) == -1                     # EINVAL: alignment
+    assert s.L.tdpd_set_workspace(s.h, C.c_void_p(base), need) == 0
+    s.workspace = buf
+    assert code(lambda: s.load_particles(pos)) == -2                                         # ESTATE: frozen
+    assert s.L.tdpd_set_workspace(s.h, C.c_void_p(base), need) == -2                         # ESTATE: twice
+    assert code(lambda: s.set_params(W.fluid_params((21, 20, 20), 3.0, seed=5, n_types=3))) == -1   # box is fixed
+    assert code(lambda: s.set_params(dict(p, dt=np.float32(0.02)))) == -1                    # dt fixed with membranes
+    assert s.L.tdpd_set_tuning(s.h, 64, 0, 0) == -2                                          # tuning after finalize
+    s.step(2)
+    g = s.get_state()
+    assert g["step"] == 2 and np.all(np.isfinite(g["force"]))
+    # an unstable state is reported, not hidden: a NaN velocity shows up as EUNSTABLE at get_state
+    bad = g["vel"].copy(); bad[0, 0] = np.nan
+    s.set_state(None, bad, None)
+    assert code(lambda: s.get_state()) == -5
+    assert T.Simulation(p).L.tdpd_step(None, 1) == -1 and s.L.tdpd_destroy(None) == -1        # null handles
