@@ -4,8 +4,8 @@
 //   a7  K-Apply: local + global area and global volume constraints (Eq 17-18) with the current step's totals (R20)
 //   a8  dihedral bending (Eq 19)
 // One launch.  A membrane is handled by `nchunk` CTAs; each stages all vertices of its membrane in shared memory
-// (unwrapped by minimum image relative to vertex 0 and stored RELATIVE to it, so the cancellation-prone volume
-// terms see coordinates of O(cell size), not O(box)), reduces area and volume redundantly in the same fixed order,
+// (unwrapped by minimum image relative to vertex 0 and stored RELATIVE to it in fp64, exactly; every edge vector is
+// the fp32 rounding of an exact difference), reduces area and volume redundantly in the same fixed order,
 // and then every thread owns one vertex and recomputes the elements incident to it ("computed 3
 // times, once per vertex thread" — no inter-thread communication, no atomics, fixed summation order).
 #include "common.cuh"
@@ -16,13 +16,18 @@ struct V3 { float x, y, z; };
 __device__ __forceinline__ V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
 __device__ __forceinline__ V3 cross3(V3 a, V3 b) { return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x}; }
 __device__ __forceinline__ float dot3(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+// vertex positions are staged in fp64: a difference of two staged vertices is then exact and is rounded ONCE to fp32
+// (relative error 6e-8 of the edge); positions rounded to fp32 relative to vertex 0 carry 2.4e-7 ABSOLUTE, which the
+// bending term (k_b / triangle height ~ 200) turns into 3e-3 in the force
+struct D3 { double x, y, z; };
+__device__ __forceinline__ V3 edge(const D3& a, const D3& b) { return {(float)(a.x - b.x), (float)(a.y - b.y), (float)(a.z - b.z)}; }
+__device__ __forceinline__ V3 tof(const D3& a) { return {(float)a.x, (float)a.y, (float)a.z}; }
 
-// minimum-image difference a - b of two wrapped coordinates, exact where fp32 allows: the operand near L is
-// shifted by -L first (exact by Sterbenz), never the small one by +L
-__device__ __forceinline__ float min_image_diff(float a, float b, float L) {
-  float d = a - b;
-  if (d > 0.5f * L) d = (a - L) - b;
-  else if (d < -0.5f * L) d = a - (b - L);
+// minimum-image difference a - b of two wrapped fp32 coordinates, exact in fp64
+__device__ __forceinline__ double min_image_diff(float a, float b, float L) {
+  double d = (double)a - (double)b;
+  if (d > 0.5 * (double)L) d -= (double)L;
+  else if (d < -0.5 * (double)L) d += (double)L;
   return d;
 }
 
@@ -41,8 +46,8 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
   const RbcDev R = A.rbcs[m];
   const MeshTemplateDev T = A.tmpls[R.tmpl];
   const int nv = T.nv, t = threadIdx.x, NT = blockDim.x, lane = t & 31, warp = t >> 5;
-  V3* sr = (V3*)smem_raw;                         // [nv] relative unwrapped positions
-  V3* sv = (V3*)(smem_raw + (size_t)nv * 12);     // [nv] velocities
+  D3* sr = (D3*)smem_raw;                         // [nv] unwrapped positions relative to vertex 0 (fp64, exact)
+  V3* sv = (V3*)(smem_raw + (size_t)nv * 24);     // [nv] velocities
 
   // ---- stage vertices (gather through slot_of_id)
   const uint32_t slot0 = A.slot_of_id[R.first_id];
@@ -53,8 +58,9 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
     float4 p = A.st.pos[slot];
     float4 l = A.st.lo[slot];
     float4 w = A.st.vel[slot];
-    sr[v] = {min_image_diff(p.x, p0.x, P.box[0]) + (l.x - l0.x), min_image_diff(p.y, p0.y, P.box[1]) + (l.y - l0.y),
-             min_image_diff(p.z, p0.z, P.box[2]) + (l.z - l0.z)};
+    sr[v] = {min_image_diff(p.x, p0.x, P.box[0]) + ((double)l.x - (double)l0.x),
+             min_image_diff(p.y, p0.y, P.box[1]) + ((double)l.y - (double)l0.y),
+             min_image_diff(p.z, p0.z, P.box[2]) + ((double)l.z - (double)l0.z)};
     sv[v] = {w.x, w.y, w.z};
   }
   __syncthreads();
@@ -62,7 +68,7 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
   // ---- a6 K-Gather in fp64 (fixed order: thread-strided partials, shuffle tree, warps in order)
   double aA = 0.0, aV = 0.0;
   for (int k = t; k < T.ntri; k += NT) {
-    V3 a = sr[T.tri[3 * k]], b = sr[T.tri[3 * k + 1]], c = sr[T.tri[3 * k + 2]];
+    D3 a = sr[T.tri[3 * k]], b = sr[T.tri[3 * k + 1]], c = sr[T.tri[3 * k + 2]];
     double ax = a.x, ay = a.y, az = a.z, bx = b.x, by = b.y, bz = b.z, cx = c.x, cy = c.y, cz = c.z;
     double ux = bx - ax, uy = by - ay, uz = bz - az, wx = cx - ax, wy = cy - ay, wz = cz - az;
     double nx = uy * wz - uz * wy, ny = uz * wx - ux * wz, nz = ux * wy - uy * wx;
@@ -93,14 +99,15 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
   const float* kp = A.kp + R.data_off;
   const float* A0t = A.A0t + R.tri_off;
   for (int v = chunk * CH + t; v < vend; v += NT) {
-    const V3 rv = sr[v], vv = sv[v];
+    const D3 rv = sr[v];
+    const V3 vv = sv[v];
     float fx = 0.f, fy = 0.f, fz = 0.f;
     const int e0 = T.voff[v], e1 = T.voff[v + 1];
     // a5 bonds (Eq 13-16): force on v from bond (v,u), d = r_v - r_u
     for (int e = e0; e < e1; ++e) {
       uint32_t pk = T.vbond[e];
       int u = pk & 0xFFFFu, b = pk >> 16;
-      V3 d = rv - sr[u], dv = vv - sv[u];
+      V3 d = edge(rv, sr[u]), dv = vv - sv[u];
       float h2 = dot3(d, d), hinv = rsqrtf(h2), h = h2 * hinv;
       V3 ev = {d.x * hinv, d.y * hinv, d.z * hinv};
       float x = h * R.inv_x0 / h0[b];
@@ -137,14 +144,15 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
       uint32_t pk = T.vtri[e];
       int tri = pk & 0xFFFFu, role = pk >> 16;
       int i1 = T.tri[3 * tri + (role + 1) % 3], i2 = T.tri[3 * tri + (role + 2) % 3];
-      V3 pa = sr[i1], pb = sr[i2];
-      V3 xi = cross3(pa - rv, pb - rv);  // same normal for any cyclic start
+      const D3 pad = sr[i1], pbd = sr[i2];
+      V3 pa = tof(pad), pb = tof(pbd);
+      V3 xi = cross3(edge(pad, rv), edge(pbd, rv));  // same normal for any cyclic start
       float l2 = dot3(xi, xi), linv = rsqrtf(l2);
       float At = 0.5f * l2 * linv;
       float a0 = A0t[tri];
       float beta = beta_g - R.k_l * (At - a0) / a0;
       V3 nh = {xi.x * linv, xi.y * linv, xi.z * linv};
-      V3 ga = cross3(nh, pb - pa), gv = cross3(pa, pb);
+      V3 ga = cross3(nh, edge(pbd, pad)), gv = cross3(pa, pb);
       fx += 0.5f * beta * ga.x + beta_v6 * gv.x;
       fy += 0.5f * beta * ga.y + beta_v6 * gv.y;
       fz += 0.5f * beta * ga.z + beta_v6 * gv.z;
@@ -153,12 +161,26 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
     for (int e = T.vdoff[v]; e < T.vdoff[v + 1]; ++e) {
       uint32_t pk = T.vdih[e];
       int q = pk & 0xFFFFu, role = pk >> 16;
-      V3 r1 = sr[T.dih[4 * q]], r2 = sr[T.dih[4 * q + 1]], r3 = sr[T.dih[4 * q + 2]], r4 = sr[T.dih[4 * q + 3]];
-      V3 xi = cross3(r2 - r1, r3 - r1), ze = cross3(r3 - r4, r2 - r4), ee = r3 - r2;
-      float xi2 = dot3(xi, xi), ze2 = dot3(ze, ze), e2 = dot3(ee, ee);
-      float ixz = rsqrtf(xi2 * ze2), le = sqrtf(e2);
-      float cth = dot3(xi, ze) * ixz;
-      float sth = dot3(cross3(xi, ze), ee) * ixz / le;
+      D3 r1 = sr[T.dih[4 * q]], r2 = sr[T.dih[4 * q + 1]], r3 = sr[T.dih[4 * q + 2]], r4 = sr[T.dih[4 * q + 3]];
+      // the two triangle normals in fp64 from the exact edge differences
+      V3 ee = edge(r3, r2);
+      double ax = r2.x - r1.x, ay = r2.y - r1.y, az = r2.z - r1.z;
+      double bx = r3.x - r1.x, by = r3.y - r1.y, bz = r3.z - r1.z;
+      double cx = r3.x - r4.x, cy = r3.y - r4.y, cz = r3.z - r4.z;
+      double dx = r2.x - r4.x, dy = r2.y - r4.y, dz = r2.z - r4.z;
+      double xid[3] = {ay * bz - az * by, az * bx - ax * bz, ax * by - ay * bx};
+      double zed[3] = {cy * dz - cz * dy, cz * dx - cx * dz, cx * dy - cy * dx};
+      double xi2d = xid[0] * xid[0] + xid[1] * xid[1] + xid[2] * xid[2];
+      double ze2d = zed[0] * zed[0] + zed[1] * zed[1] + zed[2] * zed[2];
+      double cd = xid[0] * zed[0] + xid[1] * zed[1] + xid[2] * zed[2];
+      double sd = (xid[1] * zed[2] - xid[2] * zed[1]) * ee.x + (xid[2] * zed[0] - xid[0] * zed[2]) * ee.y +
+                  (xid[0] * zed[1] - xid[1] * zed[0]) * ee.z;
+      V3 xi = {(float)xid[0], (float)xid[1], (float)xid[2]}, ze = {(float)zed[0], (float)zed[1], (float)zed[2]};
+      float xi2 = (float)xi2d, ze2 = (float)ze2d, e2 = dot3(ee, ee);
+      float le = sqrtf(e2);
+      double ixzd = rsqrt(xi2d * ze2d);
+      float cth = (float)(cd * ixzd);
+      float sth = (float)(sd * ixzd) / le;
       // sin(theta - theta0) with (cos, sin) normalised (they are, up to rounding)
       float nrm = rsqrtf(cth * cth + sth * sth);
       float coef = -R.k_b * (sth * R.cos_t0 - cth * R.sin_t0) * nrm;
@@ -167,7 +189,7 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
       if (role == 0) { w1 = 1.f; w4 = 0.f; }
       else if (role == 3) { w1 = 0.f; w4 = 1.f; }
       else {
-        float s1 = dot3(r1 - r2, ee) / e2, s4 = dot3(r4 - r2, ee) / e2;
+        float s1 = dot3(edge(r1, r2), ee) / e2, s4 = dot3(edge(r4, r2), ee) / e2;
         if (role == 1) { w1 = -(1.f - s1); w4 = -(1.f - s4); }
         else { w1 = -s1; w4 = -s4; }
       }
@@ -184,7 +206,7 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
 int td_launch_membrane(const DevParams& P, const MembraneArgs& A, int n_rbc, int max_nv, int nthreads,
                        cudaStream_t st) {
   if (n_rbc == 0) return 0;
-  size_t smem = (size_t)max_nv * 24;
+  size_t smem = (size_t)max_nv * 36;
   cudaError_t e = cudaFuncSetAttribute(k_membrane, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
   k_membrane<<<n_rbc * A.nchunk, nthreads, smem, st>>>(P, A);
