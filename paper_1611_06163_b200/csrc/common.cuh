@@ -122,20 +122,6 @@ __device__ __forceinline__ void td_box_muller_fast(uint32_t xa, uint32_t xb, flo
   g_sin = R * td_sin_approx(ang);
 }
 
-// full-precision variant (libdevice logf / sincospif, ~1 ulp) for the membrane kernel: bond random forces carry the
-// prefactor sqrt(2 kBT/dt) sqrt(2 gamma_T) ~ 35, so the 1e-5 absolute error of the MUFU path would cost 1e-3 in the
-// force of a vertex; there are only ~4 bonds per membrane vertex, so the cost is nil
-__device__ __forceinline__ void td_box_muller_precise(uint32_t xa, uint32_t xb, float& g_cos, float& g_sin) {
-  const float u = td_uniform(xa);
-  const float t = 1.0f - u;
-  const float q = t < 7.62939453125e-06f ? fmaf(t, t, t + t) : -2.0f * logf(u);
-  const float R = sqrtf(q);
-  float sn, cs;
-  sincospif(2.0f * td_uniform(xb), &sn, &cs);
-  g_cos = R * cs;
-  g_sin = R * sn;
-}
-
 // ---- kernel argument blocks -----------------------------------------------------------------------------
 struct SortedState {   // one side of the ping-pong, cell-sorted order
   float4* pos;     // x, y, z, id (bits)

@@ -124,8 +124,8 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
         uint32_t x0, x1, x2, x3;
         float g0, g1, g2, g3;
         td_philox(lo, hi, step, 1u + row, P.key0, P.key1, x0, x1, x2, x3);
-        td_box_muller_precise(x0, x1, g0, g1);
-        td_box_muller_precise(x2, x3, g2, g3);
+        td_box_muller(x0, x1, g0, g1);
+        td_box_muller(x2, x3, g2, g3);
         N[3 * row] = g0; N[3 * row + 1] = g1; N[3 * row + 2] = g2;
       }
       float tr = N[0] + N[4] + N[8];
