@@ -15,7 +15,7 @@
 //   scan      each thread walks its runs and pushes the hits, branch-free, onto a private two-ended stack of 16-bit
 //             entries (run << 11 | offset) in shared memory: front r < min(r_c, r_cc), back the ring up to
 //             max(r_c, r_cc).  85 % of the candidates are rejected here for ~14 instructions each.
-//   drain     after every run the warp pops the largest multiple of 4 (front) / 8 (back) entries that EVERY lane
+//   drain     after every run the warp pops the largest multiple of 2 (front) / 4 (back) entries that EVERY lane
 //             owns and evaluates them (Philox-4x32-10, Box-Muller, weights), two entries per iteration for
 //             instruction-level parallelism, so the expensive loops run with all lanes busy; a full stack or the
 //             end of the stencil drains everything.
@@ -32,6 +32,12 @@
 #endif
 #ifndef TD_PAIR_ILP
 #define TD_PAIR_ILP 2  // list entries evaluated per iteration
+#endif
+#ifndef TD_PAIR_BA
+#define TD_PAIR_BA 2  // drain batch of the front stack (entries; measured best of 2 / 4 / 8)
+#endif
+#ifndef TD_PAIR_BB
+#define TD_PAIR_BB 4  // drain batch of the back stack (measured best of 2 / 4 / 6 / 8 / 16)
 #endif
 #ifndef TD_PAIR_MINB
 #define TD_PAIR_MINB 3
@@ -250,7 +256,7 @@ __global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constan
     // Entries are evaluated in warp-uniform batches popped from the tops: after every scanned cell the warp takes
     // the largest multiple of BA (BB) entries that EVERY lane owns, so all lanes run the expensive loops together;
     // a lane whose stack is full, or the end of the stencil, drains everything.
-    constexpr int BA = 4, BB = 8;
+    constexpr int BA = TD_PAIR_BA, BB = TD_PAIR_BB;
     const uint32_t stride = 2u * (uint32_t)NT;
     const int sh = 31 - __clz((int)stride);
     const uint32_t lf32 = (uint32_t)__cvta_generic_to_shared(lfront), lb32 = (uint32_t)__cvta_generic_to_shared(lback);
