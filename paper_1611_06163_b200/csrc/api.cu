@@ -820,7 +820,7 @@ static int check_err_word(tdpd_sim* s) {
 
 static int fetch(tdpd_sim* s, int what, int width, float* host) {
   if (!host || s->n == 0) return TDPD_OK;
-  td_launch_unsort(s->st[s->cur], s->F4, s->Qx, s->Fb, s->n, s->prm.n_species, what, s->staging, s->err_d, s->sA);
+  td_launch_unsort(s->st[s->cur], s->F4, s->Qx, s->Fb, s->n, s->prm.n_species, what, s->staging, s->err_d, s->dp.box, s->sA);
   s->launches += 1;
   CK(cudaMemcpyAsync(host, s->staging, (size_t)s->n * width * sizeof(float), cudaMemcpyDeviceToHost, s->sA));
   CK(cudaStreamSynchronize(s->sA));

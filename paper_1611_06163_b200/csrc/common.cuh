@@ -223,7 +223,7 @@ size_t td_pair_smem_bytes(int lcap, int nthreads);
 int td_launch_membrane(const DevParams& P, const MembraneArgs& A, int n_rbc, int max_nv, int nthreads,
                        cudaStream_t st);
 void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, const float4* Fb, int64_t n,
-                      int n_species, int what, float* out, int* err, cudaStream_t st);
+                      int n_species, int what, float* out, int* err, const float* box, cudaStream_t st);
 void td_launch_set_state(const DevParams& P, const SortedState& s, int64_t n, const float* pos, const float* vel,
                          const float* conc, cudaStream_t st);
 void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, int32_t* cell_xyz,

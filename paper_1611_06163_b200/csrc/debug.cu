@@ -9,14 +9,24 @@ namespace {
 template <int S>
 __global__ void __launch_bounds__(256) k_unsort(SortedState st, const float4* __restrict__ F4,
                                                 const float* __restrict__ Qx, const float4* __restrict__ Fb, int64_t n,
-                                                int what, float* __restrict__ out, int* err) {
+                                                int what, float* __restrict__ out, int* err, float bx, float by,
+                                                float bz) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float4 p = st.pos[i];
   int64_t id = __float_as_uint(p.w);
   float v[4] = {0.f, 0.f, 0.f, 0.f};
   int cnt = 3;
-  if (what == 0) { float4 l = st.lo[i]; v[0] = p.x + l.x; v[1] = p.y + l.y; v[2] = p.z + l.z; }
+  if (what == 0) {  // hi + lo rounded to fp32, kept inside [0, L): hi = 0 with lo < 0 would round to -1e-9
+    float4 l = st.lo[i];
+    const float L[3] = {bx, by, bz};
+    v[0] = p.x + l.x; v[1] = p.y + l.y; v[2] = p.z + l.z;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      if (v[a] < 0.0f) v[a] = 0.0f;
+      if (v[a] >= L[a]) v[a] = nextafterf(L[a], 0.0f);
+    }
+  }
   else if (what == 1) { float4 w = st.vel[i]; v[0] = w.x; v[1] = w.y; v[2] = w.z; }
   else if (what == 2) {
     cnt = S;
@@ -159,14 +169,14 @@ __global__ void k_rng_debug(const DevParams P, int64_t n, const int64_t* __restr
 }  // namespace
 
 void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, const float4* Fb, int64_t n,
-                      int n_species, int what, float* out, int* err, cudaStream_t st) {
+                      int n_species, int what, float* out, int* err, const float* box, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
   switch (n_species) {
-    case 1: k_unsort<1><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err); break;
-    case 2: k_unsort<2><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err); break;
-    case 3: k_unsort<3><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err); break;
-    default: k_unsort<4><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err); break;
+    case 1: k_unsort<1><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
+    case 2: k_unsort<2><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
+    case 3: k_unsort<3><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
+    default: k_unsort<4><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
   }
 }
 
