@@ -442,10 +442,10 @@ static void build_grid(tdpd_sim* s) {
     // sub-wave systems (fewer particles than the GPU has thread slots): several threads per particle
     int split = s->n >= 300000 ? 1 : (s->n >= 20000 ? 2 : 16);
     s->pair_split = s->tune_split ? s->tune_split : split;
-    // stack capacity: ~1.9 x the mean number of neighbours (a full stack forces an early, ragged drain), at most 112
+    // stack capacity: ~1.9 x the mean number of neighbours (a full stack forces an early, ragged drain), at most 120
     // entries so that three 256-thread CTAs still fit the shared memory of an SM
     int lc = ((int)(mn * 1.9 / s->pair_split) + 8 + 1) / 2 * 2;
-    s->lcap = s->tune_lcap ? s->tune_lcap : std::min(112, std::max(16, lc));
+    s->lcap = s->tune_lcap ? s->tune_lcap : std::min(120, std::max(16, lc));
     s->pair_nt = s->tune_nt ? s->tune_nt : (s->pair_split <= 2 ? 256 : 128);
     if (s->pair_nt < s->pair_split) s->pair_nt = s->pair_split;
   }

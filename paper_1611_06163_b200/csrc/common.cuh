@@ -199,7 +199,7 @@ struct MembraneArgs {
 enum { TD_ERR_CELL_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4 };
 
 #ifndef TD_PAIR_MAXLOC
-#define TD_PAIR_MAXLOC 32  // cells per neighbour-table chunk of the pair kernel
+#define TD_PAIR_MAXLOC 24  // cells per neighbour-table chunk of the pair kernel (a 256-slot blob spans ~20)
 #endif
 
 // ---- launchers (each .cu exposes host functions; all launches are asynchronous on `st`) -------------------

@@ -25,10 +25,10 @@
 #include "common.cuh"
 
 #ifndef TD_PAIR_MAXLOC
-#define TD_PAIR_MAXLOC 32
+#define TD_PAIR_MAXLOC 24
 #endif
 #ifndef TD_PAIR_UNROLL
-#define TD_PAIR_UNROLL 4
+#define TD_PAIR_UNROLL 8  // measured best of 2 / 4 / 8 / 12 / 16 once the stacks leave no L1: 8 loads in flight per thread
 #endif
 #ifndef TD_PAIR_ILP
 #define TD_PAIR_ILP 2  // list entries evaluated per iteration
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constan
         const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
         const uint32_t room = (uint32_t)(((int)(pb - pa) >> sh) + 1);  // free entries (pa <= pb + stride always)
         const uint32_t eend = min(ecnt, e + room * SPLIT);
-#pragma unroll SCAN_UNROLL
+#pragma unroll (SPLIT == 1 ? SCAN_UNROLL : 4)
         for (; e < eend; e += SPLIT) {
           const float4 pj = __ldg(&src[e]);
           const float dx = xs - pj.x, dy = ys - pj.y, dz = zs - pj.z;
