@@ -19,7 +19,7 @@
 //             owns and evaluates them (Philox-4x32-10, Box-Muller, weights), two entries per iteration for
 //             instruction-level parallelism, so the expensive loops run with all lanes busy; a full stack or the
 //             end of the stencil drains everything.
-// Shared memory per thread is ~240 B (24 warps per SM at 80 registers); the first version staged whole halos, ran
+// Shared memory per thread is ~290 B (24 warps per SM at 80 registers); the first version staged whole halos, ran
 // 8 warps per SM and took 4.8x longer.
 #pragma once
 #include "common.cuh"
