@@ -228,7 +228,8 @@ def run_ours(args) -> dict | None:
 
     c = args.config
     w = workload(c, rank, args.random_flux == "on")
-    sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap, pair_split=args.pair_split)
+    sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap, pair_split=args.pair_split,
+                                    skin=args.skin, nlist_cap=args.nlist_cap)
     n, S = sim.n, sim.ns
     K, Wm = args.steps, max(3, args.warmup)
     state_bytes = n * (16 * 3 + 4 * max(S - 1, 0))
@@ -377,6 +378,8 @@ def main():
     ap.add_argument("--pair-threads", type=int, default=0, help="pair-kernel CTA size override (tuning)")
     ap.add_argument("--pair-split", type=int, default=0, help="pair-kernel threads per particle override (tuning)")
     ap.add_argument("--list-cap", type=int, default=0, help="pair-kernel list capacity override (tuning)")
+    ap.add_argument("--skin", type=float, default=0.0, help="neighbour-list mode: skin radius (0 = bin every step)")
+    ap.add_argument("--nlist-cap", type=int, default=0, help="neighbour-list capacity per particle (0 = automatic)")
     ap.add_argument("--random-flux", default="on", choices=["on", "off"],
                     help="off: m_s = 0, the random concentration flux dropped as in the paper (PAPER.md:78)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")

@@ -181,8 +181,9 @@ int tdpd_host_grid(const tdpd_params* p, int32_t ncell[3], uint32_t* n_runs, uin
 /* Per-kernel timing with CUDA events on the launching streams (bench.py's roofline leg).  While enabled every
  * launch of the kernels below is bracketed by an event pair; tdpd_get_timing synchronises and returns, per
  * kernel class, the number of launches and the summed milliseconds since tdpd_set_timing(s, 1).
- * Classes: 0 integrate (kick/drift/key), 1 sort, 2 reorder + cell table, 3 pair, 4 membrane, 5 closing kick. */
-#define TDPD_N_TIMERS 6
+ * Classes: 0 integrate (kick/drift/key), 1 sort, 2 reorder + cell table, 3 pair, 4 membrane, 5 closing kick,
+ * 6 neighbour list (rebuild decision + list build; neighbour-list mode only). */
+#define TDPD_N_TIMERS 7
 int tdpd_set_timing(tdpd_sim* s, int32_t on);
 int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], double ms[TDPD_N_TIMERS]);
 
@@ -194,6 +195,23 @@ int64_t tdpd_launch_count(const tdpd_sim* s);
  * per-thread neighbour list in shared memory (a full list is evaluated early, never overflowed), pair_split in
  * {1, 2, 4, 16} = threads per particle (sub-wave systems); 0 = automatic.  ESTATE after tdpd_set_workspace. */
 int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_cap, int32_t pair_split);
+
+/* the paper's own operating regime ("Neighbor lists were updated every 5 steps";
+ * construction and transposed layout PAPER.md:136-138).  skin > 0 switches the neighbour-list mode on: the cells get
+ * an edge >= max(r_c, r_cc) + skin, every binning also writes, per particle, the list of all particles within
+ * cutoff + skin (16-bit entries, [tile of 256 slots][entry][lane]), and the following steps skip sort, reorder and
+ * the 27-cell scan: the pair kernel re-tests the list entries against the true cutoffs with the current positions.
+ * After the drift of every step the device takes the largest displacement d_max since the last binning and re-bins
+ * in that same step iff 2 d_max > skin (a pair inside a cutoff could otherwise be missing), so the forces are those of
+ * the every-step binning up to the fp32 summation order.  list_cap = entries per particle (0: 1.5 x the mean + 32);
+ * a fuller neighbourhood sets an error reported by tdpd_get_state (EUNSTABLE).  skin = 0 switches the mode off.
+ * ESTATE after tdpd_set_workspace; EINVAL if the box has fewer than 3 cells of edge cutoff + skin per axis. */
+int tdpd_set_neighbor_list(tdpd_sim* s, float skin, int32_t list_cap);
+
+/* Neighbour-list mode: binnings (list rebuilds) and force evaluations since creation, the list capacity and the
+ * longest list of the last binning.  Any pointer may be NULL.  Synchronises. */
+int tdpd_get_neighbor_list_stats(tdpd_sim* s, int64_t* n_rebuilds, int64_t* n_evaluations, int32_t* list_cap,
+                                 int32_t* max_entries);
 
 /* Steps are replayed as CUDA graphs (one per ping-pong side x first/last step of a call, captured on first use) unless
  * per-kernel timing is on; on = 0 switches to plain launches.  Results are bit-identical either way. */

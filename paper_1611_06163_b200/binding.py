@@ -13,8 +13,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtdpd.so")
-MAX_TYPES, MAX_SPECIES, N_TIMERS = 4, 4, 6
-TIMER_NAMES = ("integrate", "sort", "reorder", "pair", "membrane", "closing_kick")
+MAX_TYPES, MAX_SPECIES, N_TIMERS = 4, 4, 7
+TIMER_NAMES = ("integrate", "sort", "reorder", "pair", "membrane", "closing_kick", "nlist")
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EUNSTABLE = 0, -1, -2, -3, -4, -5
 
 # every symbol include/tdpd.h declares
@@ -23,7 +23,7 @@ SYMBOLS = (
     "tdpd_set_params", "tdpd_set_state", "tdpd_step", "tdpd_sync", "tdpd_get_state", "tdpd_get_forces_split",
     "tdpd_num_particles", "tdpd_num_rbc", "tdpd_get_rbc_stats", "tdpd_get_rbc_topology", "tdpd_debug_get_binning",
     "tdpd_debug_neighbor_census", "tdpd_debug_rng", "tdpd_host_grid", "tdpd_set_timing", "tdpd_get_timing", "tdpd_launch_count",
-    "tdpd_set_tuning", "tdpd_set_graph", "tdpd_last_error", "tdpd_destroy",
+    "tdpd_set_tuning", "tdpd_set_neighbor_list", "tdpd_get_neighbor_list_stats", "tdpd_set_graph", "tdpd_last_error", "tdpd_destroy",
 )
 
 
@@ -115,6 +115,8 @@ def load_library() -> C.CDLL:
     L.tdpd_launch_count.argtypes = [vp]
     L.tdpd_launch_count.restype = i64
     L.tdpd_set_tuning.argtypes = [vp, i32, i32, i32]
+    L.tdpd_set_neighbor_list.argtypes = [vp, C.c_float, i32]
+    L.tdpd_get_neighbor_list_stats.argtypes = [vp, P(i64), P(i64), P(i32), P(i32)]
     L.tdpd_set_graph.argtypes = [vp, i32]
     L.tdpd_last_error.argtypes = [vp]
     L.tdpd_last_error.restype = C.c_char_p
@@ -154,7 +156,7 @@ class Simulation:
     """One tDPD + RBC simulation on one GPU.  Methods mirror the C ABI one to one."""
 
     def __init__(self, params: dict, device: int = 0, pair_threads: int = 0, list_cap: int = 0,
-                 pair_split: int = 0):
+                 pair_split: int = 0, skin: float = 0.0, nlist_cap: int = 0):
         import torch
 
         self.L = load_library()
@@ -167,7 +169,7 @@ class Simulation:
         self._P = make_params(params)
         with torch.cuda.device(self.device):
             self.stream_pair = torch.cuda.Stream(device=self.device)
-            self.stream_bonded = torch.cuda.Stream(device=self.device)
+            self.stream_bonded = torch.cuda.Stream(device=self.device, priority=-1)  # membrane kernel first
         h = C.c_void_p()
         rc = self.L.tdpd_create(C.byref(self._P), self.device, C.c_void_p(self.stream_pair.cuda_stream),
                                 C.c_void_p(self.stream_bonded.cuda_stream), C.byref(h))
@@ -178,6 +180,8 @@ class Simulation:
         self._ntri = []
         if pair_threads or list_cap or pair_split:
             self._ck(self.L.tdpd_set_tuning(self.h, pair_threads, list_cap, pair_split))
+        if skin or nlist_cap:
+            self._ck(self.L.tdpd_set_neighbor_list(self.h, float(skin), int(nlist_cap)))
 
     def _ck(self, rc):
         if rc != OK:
@@ -315,6 +319,11 @@ class Simulation:
         g = np.zeros((len(id_i), 4), np.float32)
         self._ck(self.L.tdpd_debug_rng(self.h, len(id_i), _ptr(id_i), _ptr(id_j), step, tag, _ptr(w), _ptr(g)))
         return w, g
+
+    def neighbor_list_stats(self) -> dict:
+        a, b, c, d = C.c_int64(0), C.c_int64(0), C.c_int32(0), C.c_int32(0)
+        self._ck(self.L.tdpd_get_neighbor_list_stats(self.h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
+        return dict(rebuilds=int(a.value), evaluations=int(b.value), list_cap=int(c.value), max_entries=int(d.value))
 
     def set_graph(self, on: bool):
         self._ck(self.L.tdpd_set_graph(self.h, int(on)))

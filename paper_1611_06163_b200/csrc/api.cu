@@ -72,7 +72,13 @@ struct tdpd_sim {
   float4 *F4 = nullptr, *Fb = nullptr;
   float *Qx = nullptr, *staging = nullptr;
   int* err_d = nullptr;
-  uint32_t* step_d = nullptr;  // device copy of the step word (the integrator bumps it)
+  uint32_t* step_d = nullptr;  // device control block; word 0 = the step word (the integrator bumps it), see TD_CTL_*
+  // neighbour list reused between binnings; nl_skin > 0 switches the mode on
+  float nl_skin = 0.0f;
+  int nl_cap = 0, tune_nl_cap = 0;
+  uint16_t* nlist_d = nullptr;
+  uint32_t *nl_cnt_d = nullptr, *okey_d = nullptr;
+  float4* P4ref_d = nullptr;
   double* stats_d = nullptr;
   RbcDev* rbcs_d = nullptr;
   MeshTemplateDev* tmpls_d = nullptr;
@@ -129,10 +135,11 @@ bool validate_params(const tdpd_params* p, std::string& why) {
   return true;
 }
 
-void derive_params(const tdpd_params& p, DevParams& d) {
+// skin > 0 (neighbour-list mode): the cells must hold every pair within cutoff + skin in the 27-cell stencil
+void derive_params(const tdpd_params& p, DevParams& d, float skin = 0.0f) {
   memset(&d, 0, sizeof d);
   d.n_types = p.n_types; d.n_species = p.n_species;
-  double rcut = std::max(p.r_c, p.r_cc);
+  double rcut = (double)std::max(p.r_c, p.r_cc) + (double)skin;
   for (int a = 0; a < 3; ++a) {
     d.box[a] = p.box[a];
     d.ncell[a] = (int)std::floor((double)p.box[a] / rcut);
@@ -161,15 +168,14 @@ void derive_params(const tdpd_params& p, DevParams& d) {
       d.a[k] = p.a[i][j]; d.gamma[k] = p.gamma[i][j]; d.s_R[k] = p.s_R[i][j];
       d.sig[k] = (float)(std::sqrt(2.0 * (double)p.kBT * (double)p.gamma[i][j]) * isdt);
       if (i < p.n_types && j < p.n_types && p.s_R[i][j] != 0.5f) fast = false;
-      for (int sp = 0; sp < TD_S; ++sp) d.kappa[sp][k] = p.kappa[sp][i][j];
+      for (int sp = 0; sp < p.n_species; ++sp) d.kappa[sp][k] = p.kappa[sp][i][j];  // padded species stay 0
     }
-  for (int sp = 0; sp < TD_S; ++sp) {
+  for (int sp = 0; sp < p.n_species; ++sp) {
     d.s_c[sp] = p.s_c[sp];
     d.epsc[sp] = (float)((double)p.m_s[sp] * (double)p.m_s[sp] * (double)p.rho / (double)p.dt);
-    if (sp < p.n_species) {
-      if (p.s_c[sp] != 2.0f) fast = false;
-      if (p.m_s[sp] != 0.0f) rnd = true;
-    }
+    d.epsc2[sp] = (float)(-2.0 * std::log(2.0) * (double)p.m_s[sp] * (double)p.m_s[sp] * (double)p.rho / (double)p.dt);
+    if (p.s_c[sp] != 2.0f) fast = false;
+    if (p.m_s[sp] != 0.0f) rnd = true;
   }
   d.body_mode = p.body_mode;
   uint32_t k0 = (uint32_t)(p.seed & 0xffffffffu), k1 = (uint32_t)(p.seed >> 32);
@@ -262,8 +268,10 @@ extern "C" int tdpd_create(const tdpd_params* p, int device, void* stream_pair, 
     s->sA = (cudaStream_t)stream_pair; s->sB = (cudaStream_t)stream_bonded;
   } else {
     s->own_streams = true;
+    int plo = 0, phi = 0;
+    cudaDeviceGetStreamPriorityRange(&plo, &phi);
     if (cudaStreamCreateWithFlags(&s->sA, cudaStreamNonBlocking) != cudaSuccess ||
-        cudaStreamCreateWithFlags(&s->sB, cudaStreamNonBlocking) != cudaSuccess) { delete s; return TDPD_ECUDA; }
+        cudaStreamCreateWithPriority(&s->sB, cudaStreamNonBlocking, phi) != cudaSuccess) { delete s; return TDPD_ECUDA; }
   }
   if (cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming) != cudaSuccess) { delete s; return TDPD_ECUDA; }
@@ -449,6 +457,23 @@ static void build_grid(tdpd_sim* s) {
     s->pair_nt = s->tune_nt ? s->tune_nt : (s->pair_split <= 2 ? 256 : 128);
     if (s->pair_nt < s->pair_split) s->pair_nt = s->pair_split;
   }
+  if (s->nl_skin > 0.0f) {
+    // neighbour-list mode: one thread per particle (the list columns are per slot), list capacity ~1.5 x the mean
+    // number of particles within cutoff + skin (a full column raises TD_ERR_LIST_OVERFLOW, never overflows)
+    double rl = std::max(s->prm.r_c, s->prm.r_cc) + (double)s->nl_skin;
+    double mn = 4.18879 * rl * rl * rl * (double)s->n / ((double)s->prm.box[0] * s->prm.box[1] * s->prm.box[2]);
+    // next to a membrane both of its sheets add their vertices (surface density nv / A0) inside the list sphere
+    double mv = 0.0;
+    for (auto& R : s->rbcs) mv = std::max(mv, 2.0 * 3.14159265 * rl * rl * (double)R.nv / R.A0);
+    s->nl_cap = s->tune_nl_cap ? s->tune_nl_cap : ((int)(1.5 * mn + 1.25 * mv) + 32 + 7) / 8 * 8;
+    s->pair_split = 1;
+    s->pair_nt = 256;
+    if (!s->tune_lcap) {
+      double rcut = std::max(s->prm.r_c, s->prm.r_cc);
+      double m0 = 4.18879 * rcut * rcut * rcut * (double)s->n / ((double)s->prm.box[0] * s->prm.box[1] * s->prm.box[2]);
+      s->lcap = std::min(120, std::max(16, ((int)(m0 * 1.9) + 8 + 1) / 2 * 2));
+    }
+  }
   // membrane kernel: CTAs per membrane so that small suspensions still fill the machine
   int M = (int)s->rbcs.size();
   if (M) {
@@ -491,8 +516,8 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->seg_first_d = c.take<uint32_t>(s->seg_first.size());
   s->seg_meta_d = c.take<uint32_t>(s->seg_meta.size());
   s->rec.P4 = c.take<float4>(n);
-  s->rec.X4 = c.take<float4>(n);
-  s->rec.Y2 = c.take<float2>(S > 2 ? n : 1);
+  s->rec.R8 = c.take<float4>(2 * n);
+  s->rec.Y4 = c.take<float4>(std::max<size_t>(1, n * (size_t)td_species_groups(S)));
   s->slot_of_id = c.take<uint32_t>(n);
   s->F4 = c.take<float4>(n);
   s->Fb = c.take<float4>(n);
@@ -500,6 +525,12 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->staging = c.take<float>(n * 4 * 3);  // up to three id-ordered arrays of <= 4 floats per particle
   s->err_d = c.take<int>(64);
   s->step_d = c.take<uint32_t>(64);
+  if (s->nl_skin > 0.0f) {
+    s->okey_d = c.take<uint32_t>(n);
+    s->P4ref_d = c.take<float4>(n);
+    s->nl_cnt_d = c.take<uint32_t>(n);
+    s->nlist_d = c.take<uint16_t>(((n + 255) / 256) * (size_t)s->nl_cap * 256);
+  }
   size_t M = s->rbcs.size();
   s->stats_d = c.take<double>(2 * std::max<size_t>(M, 1));
   s->rbcs_d = c.take<RbcDev>(std::max<size_t>(M, 1));
@@ -646,29 +677,66 @@ struct Scope {  // optional event pair around a group of launches on one stream
   ~Scope() { if (e1) cudaEventRecord(e1, q); }
 };
 
+PairArgs pair_args(tdpd_sim* s, int c) {
+  PairArgs A;
+  A.rec = s->rec; A.vel = s->st[c].vel; A.pos = s->st[c].pos; A.lo = s->st[c].lo;
+  A.keys = s->nl_skin > 0.0f ? s->okey_d : s->keys_sorted;
+  A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
+  A.seg_off = s->seg_off_d; A.seg_first = s->seg_first_d; A.seg_meta = s->seg_meta_d;
+  A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step_p = s->step_d; A.lcap = s->lcap; A.err = s->err_d;
+  A.nlist = s->nlist_d; A.nl_cnt = s->nl_cnt_d; A.nl_cap = s->nl_cap;
+  const float rl = std::max(s->prm.r_c, s->prm.r_cc) + s->nl_skin;
+  A.rlist2 = rl * rl;
+  return A;
+}
+
 int bin_and_sort(tdpd_sim* s, int mode /*0 keys only, 1 open, 2 close+open*/) {
-  const int c = s->cur;
+  const bool lm = s->nl_skin > 0.0f;
+  const int c = s->cur;  // neighbour-list mode: always side 0
+  ListRefresh LR = {s->okey_d, s->rank_cell_d, s->rec, s->P4ref_d};
   {
     Scope t(s, 0, s->sA);
     if (mode == 0) td_launch_init_keys(s->dp, s->st[c], s->n, s->keys[0], s->vals[0], s->cell_rank_d, s->sA);
     else td_launch_kick_drift_key(s->dp, s->st[c], s->F4, s->Qx, s->Fb, s->n, s->keys[0], s->vals[0], s->cell_rank_d,
-                                  mode == 2, s->step_d, s->sA);
+                                  mode == 2, s->step_d, lm ? &LR : nullptr, s->sA);
     s->launches += 1; s->timers[0].launches += 1;
+  }
+  const uint32_t* gate = nullptr;
+  if (lm) {  // the device decides whether this step re-bins; the binning kernels below return at once if not
+    Scope t(s, 6, s->sA);
+    if (mode == 0) {  // first evaluation / after set_state: positions are new, bin unconditionally
+      static const uint32_t one = 1u;
+      CK(cudaMemcpyAsync(s->step_d + TD_CTL_FORCE, &one, 4, cudaMemcpyHostToDevice, s->sA));
+    }
+    td_launch_list_decide(s->step_d, s->nl_skin * s->nl_skin, s->sA);
+    s->launches += 1; s->timers[6].launches += 1;
+    gate = s->step_d;
   }
   int side, nl = 0;
   {
     Scope t(s, 1, s->sA);
-    side = td_launch_sort(s->keys, s->vals, s->n, s->key_bits, s->sort_scratch, s->sA, &nl);
+    side = td_launch_sort(s->keys, s->vals, s->n, s->key_bits, s->sort_scratch, s->sA, &nl, gate);
     s->launches += nl; s->timers[1].launches += nl;
   }
   {
     Scope t(s, 2, s->sA);
     td_launch_reorder(s->dp, s->st[c], s->st[c ^ 1], s->rec, s->keys[side], s->vals[side], s->rank_cell_d, s->n,
-                      s->ncells, s->cell_start, s->slot_of_id, s->sA);
+                      s->ncells, s->cell_start, s->slot_of_id, lm ? s->okey_d : nullptr, s->P4ref_d, gate, s->sA);
     s->keys_sorted = s->keys[side];
     s->launches += 1; s->timers[2].launches += 1;
+    if (lm && s->n) {  // the state stays on side 0
+      td_launch_copy_state(s->dp, s->st[c ^ 1], s->st[c], s->n, gate, s->sA);
+      s->launches += 1; s->timers[2].launches += 1;
+    }
   }
-  s->cur = c ^ 1;
+  if (lm) {
+    Scope t(s, 6, s->sA);
+    int rc = td_launch_build_list(s->dp, pair_args(s, c), gate, s->sA);
+    if (rc) return fail(s, TDPD_ECUDA, std::string("list kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
+    if (s->n) { s->launches += 1; s->timers[6].launches += 1; }
+  } else {
+    s->cur = c ^ 1;
+  }
   s->binned = true;
   CK(cudaGetLastError());
   return TDPD_OK;
@@ -677,22 +745,12 @@ int bin_and_sort(tdpd_sim* s, int mode /*0 keys only, 1 open, 2 close+open*/) {
 int eval_forces(tdpd_sim* s) {
   const int c = s->cur;
   const bool mem = !s->rbcs.empty();
+  // the membrane kernel (stream B) is enqueued BEFORE the pair kernel: its few CTAs take their SM slots at once and
+  // the pair grid fills the rest; enqueued after it, they only got slots as the pair grid drained (0.15 ms of the
+  // step in round 1).  The binding also gives stream B the higher priority.
   if (mem) {
     CK(cudaEventRecord(s->ev_fork, s->sA));
     CK(cudaStreamWaitEvent(s->sB, s->ev_fork, 0));
-  }
-  {
-    Scope t(s, 3, s->sA);
-    PairArgs A;
-    A.rec = s->rec; A.vel = s->st[c].vel; A.pos = s->st[c].pos; A.lo = s->st[c].lo; A.keys = s->keys_sorted;
-    A.cell_start = s->cell_start; A.cell_rank = s->cell_rank_d; A.rank_cell = s->rank_cell_d;
-    A.seg_off = s->seg_off_d; A.seg_first = s->seg_first_d; A.seg_meta = s->seg_meta_d;
-    A.F4 = s->F4; A.Qx = s->Qx; A.n = s->n; A.step_p = s->step_d; A.lcap = s->lcap; A.err = s->err_d;
-    int rc = td_launch_pair(s->dp, A, s->pair_nt, s->pair_split, s->sA);
-    if (rc) return fail(s, TDPD_ECUDA, std::string("pair kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
-    s->launches += 1; s->timers[3].launches += 1;
-  }
-  if (mem) {
     {
       Scope t(s, 4, s->sB);
       MembraneArgs M;
@@ -704,8 +762,14 @@ int eval_forces(tdpd_sim* s) {
       s->launches += 1; s->timers[4].launches += 1;
     }
     CK(cudaEventRecord(s->ev_join, s->sB));
-    CK(cudaStreamWaitEvent(s->sA, s->ev_join, 0));
   }
+  {
+    Scope t(s, 3, s->sA);
+    int rc = td_launch_pair(s->dp, pair_args(s, c), s->pair_nt, s->pair_split, s->nl_skin > 0.0f, s->sA);
+    if (rc) return fail(s, TDPD_ECUDA, std::string("pair kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
+    s->launches += 1; s->timers[3].launches += 1;
+  }
+  if (mem) CK(cudaStreamWaitEvent(s->sA, s->ev_join, 0));
   CK(cudaGetLastError());
   s->have_forces = true;
   return TDPD_OK;
@@ -784,7 +848,7 @@ extern "C" int tdpd_step(tdpd_sim* s, int32_t nsteps) {
       s->cur = side;     // the capture advanced the host bookkeeping; the launch below does it again
     }
     CK(cudaGraphLaunch(ge, s->sA));
-    s->cur = side ^ 1;
+    s->cur = s->nl_skin > 0.0f ? side : side ^ 1;  // neighbour-list mode keeps the state on one side
     s->keys_sorted = s->gkeys[side][first][last];
     s->launches += s->glaunches[side][first][last];
     s->binned = true; s->have_forces = true;
@@ -810,7 +874,8 @@ static int check_err_word(tdpd_sim* s) {
     int zero = 0;
     cudaMemcpy(s->err_d, &zero, sizeof zero, cudaMemcpyHostToDevice);
     std::string m;
-    if (w & TD_ERR_CELL_OVERFLOW) m += "pair kernel: a cell holds more than 2047 particles; ";
+    if (w & TD_ERR_CELL_OVERFLOW) m += "pair kernel: a run of neighbour cells (up to 8 cells) holds more than 2047 particles; ";
+    if (w & TD_ERR_LIST_OVERFLOW) m += "neighbour list: a particle has more neighbours within cutoff + skin than the list capacity (raise list_cap in tdpd_set_neighbor_list); ";
     if (w & TD_ERR_NONFINITE) m += "non-finite value in the state; ";
     if (w & TD_ERR_BOND_OVERSTRETCH) m += "a WLC bond reached x >= 1; ";
     return fail(s, TDPD_EUNSTABLE, m);
@@ -897,7 +962,7 @@ extern "C" int tdpd_set_params(tdpd_sim* s, const tdpd_params* p) {
   std::string why;
   if (!validate_params(p, why)) return fail(s, TDPD_EINVAL, why);
   DevParams d;
-  derive_params(*p, d);
+  derive_params(*p, d, s->nl_skin);
   if (s->finalized) {
     if (p->n_types != s->prm.n_types || p->n_species != s->prm.n_species ||
         memcmp(d.ncell, s->dp.ncell, sizeof d.ncell) || memcmp(d.box, s->dp.box, sizeof d.box))
@@ -940,6 +1005,7 @@ extern "C" int tdpd_set_state(tdpd_sim* s, const float* pos, const float* vel, c
 extern "C" int tdpd_debug_get_binning(tdpd_sim* s, int32_t* cell_xyz, int32_t ncell[3], int32_t* cell_count,
                                       int32_t* sorted_id) {
   if (!s) return TDPD_EINVAL;
+  if (s->nl_skin > 0.0f) s->have_forces = false;  // neighbour-list mode: the slots may be those of an older binning
   int rc = ensure_forces(s);
   if (rc) return rc;
   if ((rc = tdpd_sync(s))) return rc;
@@ -964,6 +1030,7 @@ extern "C" int tdpd_debug_get_binning(tdpd_sim* s, int32_t* cell_xyz, int32_t nc
 extern "C" int tdpd_debug_neighbor_census(tdpd_sim* s, int32_t* n_rc, int32_t* n_rcc, uint32_t* xor_rc,
                                           uint32_t* xor_rcc) {
   if (!s || !n_rc || !n_rcc || !xor_rc || !xor_rcc) return TDPD_EINVAL;
+  if (s->nl_skin > 0.0f) s->have_forces = false;  // re-bin: the census walks the cell table
   int rc = ensure_forces(s);
   if (rc) return rc;
   if ((rc = tdpd_sync(s))) return rc;
@@ -1062,6 +1129,45 @@ extern "C" int tdpd_set_tuning(tdpd_sim* s, int32_t pair_threads, int32_t list_c
   s->tune_nt = pair_threads;
   s->tune_split = pair_split;
   s->tune_lcap = list_cap;
+  return TDPD_OK;
+}
+
+extern "C" int tdpd_set_neighbor_list(tdpd_sim* s, float skin, int32_t list_cap) {
+  if (!s) return TDPD_EINVAL;
+  if (s->finalized) return fail(s, TDPD_ESTATE, "the neighbour-list mode must be chosen before tdpd_set_workspace");
+  if (!(skin >= 0.0f) || list_cap < 0 || list_cap > 4096) return fail(s, TDPD_EINVAL, "skin >= 0 and 0 <= list_cap <= 4096");
+  if (skin > 0.0f) {
+    double rl = (double)std::max(s->prm.r_c, s->prm.r_cc) + (double)skin;
+    for (int a = 0; a < 3; ++a)
+      if ((int)std::floor((double)s->prm.box[a] / rl) < 3)
+        return fail(s, TDPD_EINVAL, "box smaller than 3 cells of edge cutoff + skin per axis");
+  }
+  s->nl_skin = skin;
+  s->tune_nl_cap = list_cap;
+  derive_params(s->prm, s->dp, skin);
+  s->seg_off.clear();  // the grid changed: rebuild the static neighbour runs
+  return TDPD_OK;
+}
+
+extern "C" int tdpd_get_neighbor_list_stats(tdpd_sim* s, int64_t* n_rebuilds, int64_t* n_evaluations, int32_t* list_cap,
+                                            int32_t* max_entries) {
+  if (!s) return TDPD_EINVAL;
+  if (n_rebuilds) *n_rebuilds = 0;
+  if (n_evaluations) *n_evaluations = 0;
+  if (list_cap) *list_cap = s->nl_cap;
+  if (max_entries) *max_entries = 0;
+  if (!(s->nl_skin > 0.0f) || !s->finalized) return TDPD_OK;
+  int rc = tdpd_sync(s);
+  if (rc) return rc;
+  uint32_t w[8];
+  CK(cudaMemcpy(w, s->step_d, sizeof w, cudaMemcpyDeviceToHost));
+  if (n_rebuilds) *n_rebuilds = w[TD_CTL_NREBUILD];
+  if (n_evaluations) *n_evaluations = w[TD_CTL_NDECIDE];
+  if (max_entries && s->n) {
+    std::vector<uint32_t> c((size_t)s->n);
+    CK(cudaMemcpy(c.data(), s->nl_cnt_d, (size_t)s->n * 4, cudaMemcpyDeviceToHost));
+    *max_entries = (int32_t)*std::max_element(c.begin(), c.end());
+  }
   return TDPD_OK;
 }
 

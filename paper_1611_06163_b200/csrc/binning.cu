@@ -12,8 +12,14 @@ constexpr int TILE = SORT_NT * SORT_ITEMS;
 constexpr int WCHUNK = 32 * SORT_ITEMS;  // contiguous keys owned by one warp
 
 // per-tile digit histogram -> hist[bin * nblk + blk]  (integer counts: atomics cannot change the result)
+// `gate` (may be NULL): the device control block of the neighbour-list mode; the kernels of the binning return at once
+// when this step does not re-bin (TD_CTL_REBUILD == 0), so that the launch sequence of a step stays static (CUDA graph)
+#define TD_GATE(gate) if ((gate) && (gate)[TD_CTL_REBUILD] == 0u) return
+
 __global__ void __launch_bounds__(SORT_NT) k_sort_hist(const uint32_t* __restrict__ keys, int64_t n, int shift,
-                                                       uint32_t* __restrict__ hist, int nblk) {
+                                                       uint32_t* __restrict__ hist, int nblk,
+                                                       const uint32_t* __restrict__ gate) {
+  TD_GATE(gate);
   __shared__ uint32_t cnt[NBIN];
   cnt[threadIdx.x] = 0;
   __syncthreads();
@@ -55,7 +61,8 @@ __device__ __forceinline__ uint32_t block_excl_scan_1024(uint32_t tsum, uint32_t
 }
 
 __global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ hist, int64_t total,
-                                                    uint32_t* __restrict__ tops) {
+                                                    uint32_t* __restrict__ tops, const uint32_t* __restrict__ gate) {
+  TD_GATE(gate);
   __shared__ uint32_t wsum[32];
   int64_t i0 = (int64_t)blockIdx.x * SCAN_CHUNK + (int64_t)threadIdx.x * 4;
   uint32_t v[4];
@@ -71,7 +78,9 @@ __global__ void __launch_bounds__(1024) k_sort_scan(uint32_t* __restrict__ hist,
   if (threadIdx.x == 0) tops[blockIdx.x] = gridDim.x == 1 ? 0u : sum;  // a single chunk needs no second level
 }
 
-__global__ void __launch_bounds__(1024) k_sort_scan_tops(uint32_t* __restrict__ tops, int nchunk) {
+__global__ void __launch_bounds__(1024) k_sort_scan_tops(uint32_t* __restrict__ tops, int nchunk,
+                                                         const uint32_t* __restrict__ gate) {
+  TD_GATE(gate);
   __shared__ uint32_t wsum[32];
   __shared__ uint32_t carry_s;
   if (threadIdx.x == 0) carry_s = 0;
@@ -94,7 +103,9 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
                                                           const uint32_t* __restrict__ vin,
                                                           uint32_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                           int64_t n, int shift, const uint32_t* __restrict__ hist,
-                                                          int nblk, const uint32_t* __restrict__ tops) {
+                                                          int nblk, const uint32_t* __restrict__ tops,
+                                                          const uint32_t* __restrict__ gate) {
+  TD_GATE(gate);
   __shared__ uint32_t wbase[SORT_NT / 32][NBIN];
   int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int k = threadIdx.x; k < (SORT_NT / 32) * NBIN; k += SORT_NT) (&wbase[0][0])[k] = 0;
@@ -146,7 +157,10 @@ template <int S>
 __global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState src, SortedState dst, PairRec rec,
                                                  const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
                                                  const uint32_t* __restrict__ rank_cell, int64_t n, uint32_t ncell,
-                                                 uint32_t* __restrict__ cell_start, uint32_t* __restrict__ slot_of_id) {
+                                                 uint32_t* __restrict__ cell_start, uint32_t* __restrict__ slot_of_id,
+                                                 uint32_t* __restrict__ okey, float4* __restrict__ P4ref,
+                                                 const uint32_t* __restrict__ gate) {
+  TD_GATE(gate);
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   uint32_t k = keys[i];
@@ -158,7 +172,9 @@ __global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState 
   dst.pos[i] = p;
   dst.vel[i] = v;
   dst.lo[i] = l;
-  float cxv[3] = {0.f, 0.f, 0.f};
+  float cxv[TD_S - 1];
+#pragma unroll
+  for (int s = 1; s < TD_S; ++s) cxv[s - 1] = 0.f;
 #pragma unroll
   for (int s = 1; s < S; ++s) {
     cxv[s - 1] = src.cx[(int64_t)(s - 1) * n + from];
@@ -167,10 +183,16 @@ __global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState 
   const uint32_t pc = __ldg(&rank_cell[k]);
   const float ox = (float)(pc & 1022u) * P.edge_q[0], oy = (float)((pc >> 10) & 1022u) * P.edge_q[1],
               oz = (float)((pc >> 20) & 1022u) * P.edge_q[2];  // origin of the 2x2x2 block
-  rec.P4[i] = make_float4(__fadd_rn(__fsub_rn(p.x, ox), l.x), __fadd_rn(__fsub_rn(p.y, oy), l.y),
-                          __fadd_rn(__fsub_rn(p.z, oz), l.z), p.w);
-  rec.X4[i] = make_float4(v.w, cxv[0], l.w, 0.0f);
-  if (S > 2) rec.Y2[i] = make_float2(cxv[1], cxv[2]);
+  const float4 rel = make_float4(__fadd_rn(__fsub_rn(p.x, ox), l.x), __fadd_rn(__fsub_rn(p.y, oy), l.y),
+                                 __fadd_rn(__fsub_rn(p.z, oz), l.z), p.w);
+  rec.P4[i] = rel;
+  if (okey) { okey[i] = k; P4ref[i] = rel; }  // neighbour-list mode: the binning every later step refers to
+  const float4 xr = make_float4(v.w, cxv[0], __uint_as_float(m & 3u), __uint_as_float(m >> 2));
+  rec.R8[2 * i] = rel;
+  rec.R8[2 * i + 1] = xr;
+#pragma unroll
+  for (int g = 0; g < td_species_groups(S); ++g)
+    rec.Y4[(size_t)g * n + i] = make_float4(cxv[1 + 4 * g], cxv[2 + 4 * g], cxv[3 + 4 * g], cxv[4 + 4 * g]);
   if (m >> 2) slot_of_id[__float_as_uint(p.w)] = (uint32_t)i;
   // cell_start[r] = first slot whose key >= r
   uint32_t kprev = i == 0 ? 0u : keys[i - 1] + 1u;
@@ -178,6 +200,19 @@ __global__ void __launch_bounds__(256) k_reorder(const DevParams P, SortedState 
     for (uint32_t r = kprev; r <= k; ++r) cell_start[r] = (uint32_t)i;
   if (i == n - 1)
     for (uint32_t r = k + 1; r <= ncell; ++r) cell_start[r] = (uint32_t)n;
+}
+// neighbour-list mode keeps the state on one side: the gathered copy goes back to where the integrator works
+template <int S>
+__global__ void __launch_bounds__(256) k_copy_state(SortedState src, SortedState dst, int64_t n,
+                                                    const uint32_t* __restrict__ gate) {
+  TD_GATE(gate);
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  dst.pos[i] = src.pos[i];
+  dst.vel[i] = src.vel[i];
+  dst.lo[i] = src.lo[i];
+#pragma unroll
+  for (int s = 1; s < S; ++s) dst.cx[(int64_t)(s - 1) * n + i] = src.cx[(int64_t)(s - 1) * n + i];
 }
 }  // namespace
 
@@ -191,7 +226,7 @@ size_t td_sort_scratch_bytes(int64_t n) {
 }
 
 int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits, void* scratch, cudaStream_t st,
-                   int* n_launches) {
+                   int* n_launches, const uint32_t* gate) {
   int side = 0;
   if (n == 0) return side;
   int nblk = (int)((n + TILE - 1) / TILE);
@@ -202,11 +237,11 @@ int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits
   int passes = td_sort_passes(key_bits);
   for (int p = 0; p < passes; ++p) {
     int shift = p * RB;
-    k_sort_hist<<<nblk, SORT_NT, 0, st>>>(keys[side], n, shift, hist, nblk);
-    k_sort_scan<<<nchunk, 1024, 0, st>>>(hist, nh, tops);
-    if (nchunk > 1) k_sort_scan_tops<<<1, 1024, 0, st>>>(tops, nchunk);
+    k_sort_hist<<<nblk, SORT_NT, 0, st>>>(keys[side], n, shift, hist, nblk, gate);
+    k_sort_scan<<<nchunk, 1024, 0, st>>>(hist, nh, tops, gate);
+    if (nchunk > 1) k_sort_scan_tops<<<1, 1024, 0, st>>>(tops, nchunk, gate);
     k_sort_scatter<<<nblk, SORT_NT, 0, st>>>(keys[side], vals[side], keys[side ^ 1], vals[side ^ 1], n, shift, hist,
-                                              nblk, tops);
+                                              nblk, tops, gate);
     side ^= 1;
     if (n_launches) *n_launches += nchunk > 1 ? 4 : 3;
   }
@@ -215,13 +250,17 @@ int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits
 
 void td_launch_reorder(const DevParams& P, const SortedState& src, const SortedState& dst, const PairRec& rec,
                        const uint32_t* keys, const uint32_t* vals, const uint32_t* rank_cell, int64_t n,
-                       uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, cudaStream_t st) {
+                       uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, uint32_t* okey, float4* P4ref,
+                       const uint32_t* gate, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
-  switch (P.n_species) {
-    case 1: k_reorder<1><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
-    case 2: k_reorder<2><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
-    case 3: k_reorder<3><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
-    default: k_reorder<4><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start, slot_of_id); break;
-  }
+  TD_SWITCH_S(P.n_species, k_reorder<S_><<<nb, 256, 0, st>>>(P, src, dst, rec, keys, vals, rank_cell, n, ncell, cell_start,
+                                                             slot_of_id, okey, P4ref, gate));
+}
+
+void td_launch_copy_state(const DevParams& P, const SortedState& src, const SortedState& dst, int64_t n,
+                          const uint32_t* gate, cudaStream_t st) {
+  if (n == 0) return;
+  int nb = (int)((n + 255) / 256);
+  TD_SWITCH_S(P.n_species, k_copy_state<S_><<<nb, 256, 0, st>>>(src, dst, n, gate));
 }

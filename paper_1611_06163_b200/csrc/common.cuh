@@ -5,7 +5,7 @@
 #include <stdint.h>
 
 #define TD_T 4  // max particle types
-#define TD_S 4  // max species
+#define TD_S 10  // max species (the paper benchmarks up to N_spec = 10)
 
 // Parameters in the form the kernels consume (derived once on the host from tdpd_params).
 struct DevParams {
@@ -28,6 +28,7 @@ struct DevParams {
   float s_R[TD_T * TD_T];
   float kappa[TD_S][TD_T * TD_T];
   float epsc[TD_S];  // m_s^2 rho / dt: Q^R = sgn zeta w_RC sqrt(kappa (Ci+Cj) epsc)  (Eq 9-10)
+  float epsc2[TD_S];  // -2 ln 2 * epsc: multiplies lg2(u) so that sqrt(-2 ln u) and the amplitude share one square root
   float s_c[TD_S];
   float body[3];
   int body_mode;
@@ -133,8 +134,25 @@ struct SortedState {   // one side of the ping-pong, cell-sorted order
 // pair-kernel records, written by the reorder kernel in cell-sorted order (read-only in the pair kernel)
 struct PairRec {
   float4* P4;   // x, y, z relative to the origin of the 2x2x2 cell block, (c & ~1) * edge_q (see DevParams), id (bits)
-  float4* X4;   // C_0, C_1, td_meta (bits), 0
-  float2* Y2;   // C_2, C_3 (only when n_species > 2)
+  float4* R8;   // [2n] the record the evaluation loads with ONE 256-bit load (LDG.E.256, new on sm_100) per neighbour:
+                // R8[2i] = P4[i], R8[2i+1] = C_0, C_1, type (bits), exclusion key = membrane id + 1 or 0 (bits)
+  float4* Y4;   // [td_species_groups(S)][n]: C_2..C_5, C_6..C_9 (species-major in groups of four; zero padded)
+};
+
+// the pair kernel is compiled for 1, 2, 4, 6 and 10 species; other counts run the next larger one (a padded species has
+// kappa = 0 and C = 0: its flux is exactly zero and is never stored)
+__host__ __device__ constexpr int td_species_padded(int S) { return S <= 2 ? S : S <= 4 ? 4 : S <= 6 ? 6 : 10; }
+__host__ __device__ constexpr int td_species_groups(int S) { return S <= 2 ? 0 : (td_species_padded(S) - 2 + 3) / 4; }
+
+// device control words (one 64-word block; word 0 is the RNG step word the integrator bumps)
+enum { TD_CTL_STEP = 0, TD_CTL_REBUILD = 1, TD_CTL_DMAX2 = 2, TD_CTL_FORCE = 3, TD_CTL_NREBUILD = 4, TD_CTL_NDECIDE = 5 };
+
+// what the integrator needs to keep the pair records current between binnings (neighbour-list mode)
+struct ListRefresh {
+  const uint32_t* okey;       // [n] Morton rank of the cell each slot was binned into
+  const uint32_t* rank_cell;  // [ncell]
+  PairRec rec;
+  const float4* P4ref;        // [n] P4 at the last binning (displacement reference)
 };
 
 struct PairArgs {
@@ -157,6 +175,12 @@ struct PairArgs {
   const uint32_t* step_p;      // RNG step word (device counter, bumped by the integrator: lets a step be a CUDA graph)
   int lcap;                    // list entries per thread
   int* err;                    // device error word
+  // neighbour list reused between binnings: tiles of 256 slots, [tile][entry][lane], 16-bit
+  // entries run << 11 | offset against the cell table of the binning that built it
+  uint16_t* nlist;
+  uint32_t* nl_cnt;            // [n] entries of each slot
+  int nl_cap;                  // entries per slot
+  float rlist2;                // (max(r_c, r_cc) + skin)^2
 };
 
 // mesh template (topology shared by all membranes with the same triangle list), CSR per vertex
@@ -196,29 +220,55 @@ struct MembraneArgs {
   int* err;
 };
 
-enum { TD_ERR_CELL_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4 };
+enum { TD_ERR_CELL_OVERFLOW = 1, TD_ERR_NONFINITE = 2, TD_ERR_BOND_OVERSTRETCH = 4, TD_ERR_LIST_OVERFLOW = 8 };
 
 #ifndef TD_PAIR_MAXLOC
 #define TD_PAIR_MAXLOC 24  // cells per neighbour-table chunk of the pair kernel (a 256-slot blob spans ~20)
 #endif
+// shared memory of the pair kernel ahead of the hit stacks: run table (first slot + displacement 16 B, count 4 B per
+// run), type-pair table (a, gamma, sigma, s_R), kappa per species, runs per local cell
+__host__ __device__ constexpr size_t td_pair_table_bytes() {
+  return (size_t)TD_PAIR_MAXLOC * 27 * 20 + 16 * 16 + (size_t)TD_S * 16 * 4 + TD_PAIR_MAXLOC * 4;
+}
+
+// runs `...` with the compile-time species count S_ = ns (1..TD_S)
+#define TD_SWITCH_S(ns, ...)                                       \
+  switch (ns) {                                                    \
+    case 1: { constexpr int S_ = 1; __VA_ARGS__; } break;          \
+    case 2: { constexpr int S_ = 2; __VA_ARGS__; } break;          \
+    case 3: { constexpr int S_ = 3; __VA_ARGS__; } break;          \
+    case 4: { constexpr int S_ = 4; __VA_ARGS__; } break;          \
+    case 5: { constexpr int S_ = 5; __VA_ARGS__; } break;          \
+    case 6: { constexpr int S_ = 6; __VA_ARGS__; } break;          \
+    case 7: { constexpr int S_ = 7; __VA_ARGS__; } break;          \
+    case 8: { constexpr int S_ = 8; __VA_ARGS__; } break;          \
+    case 9: { constexpr int S_ = 9; __VA_ARGS__; } break;          \
+    default: { constexpr int S_ = 10; __VA_ARGS__; } break;        \
+  }
 
 // ---- launchers (each .cu exposes host functions; all launches are asynchronous on `st`) -------------------
 void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
                          const uint32_t* cell_rank, cudaStream_t st);
 void td_launch_kick_drift_key(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
                               const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
-                              bool closing_first, uint32_t* step_d, cudaStream_t st);
+                              bool closing_first, uint32_t* ctl, const ListRefresh* LR, cudaStream_t st);
 void td_launch_kick(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx, const float4* Fb,
                     int64_t n, cudaStream_t st);
 int td_sort_passes(int key_bits);
 size_t td_sort_scratch_bytes(int64_t n);
 // sorts (keys, vals); result ends in keys[out_side]/vals[out_side]; returns out_side
 int td_launch_sort(uint32_t* keys[2], uint32_t* vals[2], int64_t n, int key_bits, void* scratch, cudaStream_t st,
-                   int* n_launches);
+                   int* n_launches, const uint32_t* gate);
 void td_launch_reorder(const DevParams& P, const SortedState& src, const SortedState& dst, const PairRec& rec,
                        const uint32_t* keys, const uint32_t* vals, const uint32_t* rank_cell, int64_t n,
-                       uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, cudaStream_t st);
-int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, int split, cudaStream_t st);
+                       uint32_t ncell, uint32_t* cell_start, uint32_t* slot_of_id, uint32_t* okey, float4* P4ref,
+                       const uint32_t* gate, cudaStream_t st);
+void td_launch_copy_state(const DevParams& P, const SortedState& src, const SortedState& dst, int64_t n,
+                          const uint32_t* gate, cudaStream_t st);
+// neighbour-list mode (pair_list.cu): the per-step decision and the list builder
+void td_launch_list_decide(uint32_t* ctl, float skin2, cudaStream_t st);
+int td_launch_build_list(const DevParams& P, const PairArgs& A, const uint32_t* gate, cudaStream_t st);
+int td_launch_pair(const DevParams& P, const PairArgs& A, int nthreads, int split, bool from_list, cudaStream_t st);
 size_t td_pair_smem_bytes(int lcap, int nthreads);
 int td_launch_membrane(const DevParams& P, const MembraneArgs& A, int n_rbc, int max_nv, int nthreads,
                        cudaStream_t st);

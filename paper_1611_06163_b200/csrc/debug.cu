@@ -15,7 +15,9 @@ __global__ void __launch_bounds__(256) k_unsort(SortedState st, const float4* __
   if (i >= n) return;
   float4 p = st.pos[i];
   int64_t id = __float_as_uint(p.w);
-  float v[4] = {0.f, 0.f, 0.f, 0.f};
+  float v[S > 3 ? S : 3];
+#pragma unroll
+  for (int k = 0; k < (S > 3 ? S : 3); ++k) v[k] = 0.f;
   int cnt = 3;
   if (what == 0) {  // hi + lo rounded to fp32, kept inside [0, L): hi = 0 with lo < 0 would round to -1e-9
     float4 l = st.lo[i];
@@ -43,10 +45,12 @@ __global__ void __launch_bounds__(256) k_unsort(SortedState st, const float4* __
     for (int s = 1; s < S; ++s) v[s] = Qx[(int64_t)(s - 1) * n + i];
   }
   bool bad = false;
-  for (int k = 0; k < cnt; ++k) {
-    out[id * cnt + k] = v[k];
-    bad |= !isfinite(v[k]);
-  }
+#pragma unroll
+  for (int k = 0; k < (S > 3 ? S : 3); ++k)
+    if (k < cnt) {
+      out[id * cnt + k] = v[k];
+      bad |= !isfinite(v[k]);
+    }
   if (bad) atomicOr(err, TD_ERR_NONFINITE);
 }
 
@@ -172,12 +176,7 @@ void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, c
                       int n_species, int what, float* out, int* err, const float* box, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
-  switch (n_species) {
-    case 1: k_unsort<1><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
-    case 2: k_unsort<2><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
-    case 3: k_unsort<3><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
-    default: k_unsort<4><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]); break;
-  }
+  TD_SWITCH_S(n_species, k_unsort<S_><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]));
 }
 
 void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, int32_t* cell_xyz,
@@ -202,10 +201,5 @@ void td_launch_set_state(const DevParams& P, const SortedState& s, int64_t n, co
                          const float* conc, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
-  switch (P.n_species) {
-    case 1: k_set_state<1><<<nb, 256, 0, st>>>(P, s, n, pos, vel, conc); break;
-    case 2: k_set_state<2><<<nb, 256, 0, st>>>(P, s, n, pos, vel, conc); break;
-    case 3: k_set_state<3><<<nb, 256, 0, st>>>(P, s, n, pos, vel, conc); break;
-    default: k_set_state<4><<<nb, 256, 0, st>>>(P, s, n, pos, vel, conc); break;
-  }
+  TD_SWITCH_S(P.n_species, k_set_state<S_><<<nb, 256, 0, st>>>(P, s, n, pos, vel, conc));
 }

@@ -67,65 +67,108 @@ __device__ __forceinline__ void td_half_kick(const DevParams& P, float4& p, floa
 
 // mode: 0 = keys only (initial binning), 1 = opening half-kick + drift + wrap + key,
 //       2 = closing half-kick of the previous step, then mode 1, 3 = closing half-kick only
-template <int S>
+// LISTM (neighbour list reused between binnings): the particles keep the slots of the last
+// binning, so the kernel also refreshes the pair kernel's records in place (position relative to the block origin
+// of the cell the particle was binned into, unwrapped through the periodic boundary; concentrations) and takes the
+// maximum displacement since that binning, which decides on the device whether this step re-bins (k_list_decide).
+template <int S, bool LISTM>
 __global__ void __launch_bounds__(256) k_integrate(const DevParams P, SortedState st, const float4* __restrict__ F4,
                                                    const float* __restrict__ Qx, const float4* __restrict__ Fb,
                                                    int64_t n, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals,
                                                    const uint32_t* __restrict__ cell_rank, int mode,
-                                                   uint32_t* __restrict__ step_d) {
+                                                   uint32_t* __restrict__ ctl, ListRefresh LR) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  if (i == 0 && step_d) *step_d += 1u;  // the force evaluation that follows the drift uses the next step word
-  float4 p = st.pos[i];
-  if (mode != 0) {
-    float4 v = st.vel[i];
-    float4 l = st.lo[i];
-    uint32_t meta = __float_as_uint(l.w);
-    float cxv[S > 1 ? S - 1 : 1];
+  float d2 = 0.0f;
+  if (i < n) {
+    if (i == 0 && ctl) ctl[TD_CTL_STEP] += 1u;  // the force evaluation that follows the drift uses the next step word
+    float4 p = st.pos[i];
+    if (mode != 0) {
+      float4 v = st.vel[i];
+      float4 l = st.lo[i];
+      uint32_t meta = __float_as_uint(l.w);
+      float cxv[S > 1 ? S - 1 : 1];
 #pragma unroll
-    for (int s = 1; s < S; ++s) cxv[s - 1] = st.cx[(int64_t)(s - 1) * n + i];
-    if (mode >= 2) td_half_kick<S>(P, p, v, cxv, F4, Qx, Fb, meta, i, n);
-    if (mode <= 2) {
-      td_half_kick<S>(P, p, v, cxv, F4, Qx, Fb, meta, i, n);
-      td_drift(p.x, l.x, P.dt, v.x, P.box[0]);
-      td_drift(p.y, l.y, P.dt, v.y, P.box[1]);
-      td_drift(p.z, l.z, P.dt, v.z, P.box[2]);
-      st.pos[i] = p;
-      st.lo[i] = l;
+      for (int s = 1; s < S; ++s) cxv[s - 1] = st.cx[(int64_t)(s - 1) * n + i];
+      if (mode >= 2) td_half_kick<S>(P, p, v, cxv, F4, Qx, Fb, meta, i, n);
+      if (mode <= 2) {
+        td_half_kick<S>(P, p, v, cxv, F4, Qx, Fb, meta, i, n);
+        td_drift(p.x, l.x, P.dt, v.x, P.box[0]);
+        td_drift(p.y, l.y, P.dt, v.y, P.box[1]);
+        td_drift(p.z, l.z, P.dt, v.z, P.box[2]);
+        st.pos[i] = p;
+        st.lo[i] = l;
+      }
+      st.vel[i] = v;
+#pragma unroll
+      for (int s = 1; s < S; ++s) st.cx[(int64_t)(s - 1) * n + i] = cxv[s - 1];
+      if (LISTM && mode <= 2) {
+        // records of the pair kernel in the slots of the last binning: exact in fp64, rounded once (as k_reorder's)
+        const uint32_t pc = __ldg(&LR.rank_cell[__ldg(&LR.okey[i])]);
+        const double o[3] = {(double)((float)(pc & 1022u) * P.edge_q[0]), (double)((float)((pc >> 10) & 1022u) * P.edge_q[1]),
+                             (double)((float)((pc >> 20) & 1022u) * P.edge_q[2])};
+        const double xa[3] = {(double)p.x + (double)l.x, (double)p.y + (double)l.y, (double)p.z + (double)l.z};
+        const float4 r0 = __ldg(&LR.P4ref[i]);
+        const float ref[3] = {r0.x, r0.y, r0.z};
+        float rel[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          // the periodic image next to where the particle was at the binning (it moved by less than the skin)
+          double t = xa[a] - o[a];
+          const double L = (double)P.box[a];
+          t -= L * rint((t - (double)ref[a]) / L);
+          rel[a] = (float)t;
+        }
+        const float4 pr = make_float4(rel[0], rel[1], rel[2], p.w);
+        const float4 xr = make_float4(v.w, S > 1 ? cxv[0] : 0.0f, __uint_as_float(meta & 3u), __uint_as_float(meta >> 2));
+        LR.rec.P4[i] = pr;
+        LR.rec.R8[2 * i] = pr;
+        LR.rec.R8[2 * i + 1] = xr;
+#pragma unroll
+        for (int g = 0; g < td_species_groups(S); ++g) {
+          float y[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) y[k] = (2 + 4 * g + k < S) ? cxv[(2 + 4 * g + k < S) ? 1 + 4 * g + k : 0] : 0.0f;
+          LR.rec.Y4[(size_t)g * n + i] = make_float4(y[0], y[1], y[2], y[3]);
+        }
+        const float ex = rel[0] - r0.x, ey = rel[1] - r0.y, ez = rel[2] - r0.z;
+        d2 = fmaf(ez, ez, fmaf(ey, ey, ex * ex));
+      }
     }
-    st.vel[i] = v;
-#pragma unroll
-    for (int s = 1; s < S; ++s) st.cx[(int64_t)(s - 1) * n + i] = cxv[s - 1];
+    if (mode <= 2) {
+      keys[i] = td_key_of(P, p.x, p.y, p.z, cell_rank);
+      vals[i] = (uint32_t)i;
+    }
   }
-  if (mode <= 2) {
-    keys[i] = td_key_of(P, p.x, p.y, p.z, cell_rank);
-    vals[i] = (uint32_t)i;
+  if (LISTM && mode != 0 && mode <= 2) {  // maximum displacement: warp max, one integer atomicMax per warp (order-free)
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) d2 = fmaxf(d2, __shfl_xor_sync(0xffffffffu, d2, d));
+    if ((threadIdx.x & 31) == 0 && d2 > 0.0f) atomicMax(&ctl[TD_CTL_DMAX2], __float_as_uint(d2));
   }
 }
 
 static void launch_integrate(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
                              const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
-                             int mode, uint32_t* step_d, cudaStream_t st) {
+                             int mode, uint32_t* ctl, const ListRefresh* LR, cudaStream_t st) {
   if (n == 0) return;
   int nb = (int)((n + 255) / 256);
-  switch (P.n_species) {
-    case 1: k_integrate<1><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
-    case 2: k_integrate<2><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
-    case 3: k_integrate<3><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
-    default: k_integrate<4><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, step_d); break;
+  if (LR) {
+    TD_SWITCH_S(P.n_species, k_integrate<S_, true><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, ctl, *LR));
+  } else {
+    ListRefresh none = {};
+    TD_SWITCH_S(P.n_species, k_integrate<S_, false><<<nb, 256, 0, st>>>(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, mode, ctl, none));
   }
 }
 
 void td_launch_init_keys(const DevParams& P, const SortedState& s, int64_t n, uint32_t* keys, uint32_t* vals,
                          const uint32_t* cell_rank, cudaStream_t st) {
-  launch_integrate(P, s, nullptr, nullptr, nullptr, n, keys, vals, cell_rank, 0, nullptr, st);
+  launch_integrate(P, s, nullptr, nullptr, nullptr, n, keys, vals, cell_rank, 0, nullptr, nullptr, st);
 }
 void td_launch_kick_drift_key(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx,
                               const float4* Fb, int64_t n, uint32_t* keys, uint32_t* vals, const uint32_t* cell_rank,
-                              bool closing_first, uint32_t* step_d, cudaStream_t st) {
-  launch_integrate(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, closing_first ? 2 : 1, step_d, st);
+                              bool closing_first, uint32_t* ctl, const ListRefresh* LR, cudaStream_t st) {
+  launch_integrate(P, s, F4, Qx, Fb, n, keys, vals, cell_rank, closing_first ? 2 : 1, ctl, LR, st);
 }
 void td_launch_kick(const DevParams& P, const SortedState& s, const float4* F4, const float* Qx, const float4* Fb,
                     int64_t n, cudaStream_t st) {
-  launch_integrate(P, s, F4, Qx, Fb, n, nullptr, nullptr, nullptr, 3, nullptr, st);
+  launch_integrate(P, s, F4, Qx, Fb, n, nullptr, nullptr, nullptr, 3, nullptr, nullptr, st);
 }

@@ -2,5 +2,5 @@
 #include "pair_kernel.cuh"
 
 int td_launch_pair_s16(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st) {
-  return launch_split<16>(P, A, nthreads, st);
+  return launch_split<16, false>(P, A, nthreads, st);
 }

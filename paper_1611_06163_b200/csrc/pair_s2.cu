@@ -2,5 +2,5 @@
 #include "pair_kernel.cuh"
 
 int td_launch_pair_s2(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st) {
-  return launch_split<2>(P, A, nthreads, st);
+  return launch_split<2, false>(P, A, nthreads, st);
 }

@@ -2,5 +2,5 @@
 #include "pair_kernel.cuh"
 
 int td_launch_pair_s4(const DevParams& P, const PairArgs& A, int nthreads, cudaStream_t st) {
-  return launch_split<4>(P, A, nthreads, st);
+  return launch_split<4, false>(P, A, nthreads, st);
 }

@@ -554,3 +554,70 @@ def test_error_paths_of_the_boundary(T):
     s.set_state(None, bad, None)
     assert code(lambda: s.get_state()) == -5
     assert T.Simulation(p).L.tdpd_step(None, 1) == -1 and s.L.tdpd_destroy(None) == -1        # null handles
+
+
+# ---------------------------------------------------------------------------------------------------------
+# neighbour list reused over several steps.  The list mode must give the
+# forces of the every-step binning (up to the fp32 summation order): same tolerances against the oracle, with
+# rebuilds happening INSIDE the compared window.
+def _list_case(name):
+    if name == "fluid":
+        return W.make_fluid("t", (13, 11, 8), 4.0, seed=21), 0.4, 30
+    if name == "config1":
+        return W.config(1), 0.4, 100
+    if name == "suspension":
+        return W.small_suspension(seed=8, box=(20, 20, 12), n_rbc=1, n_species=2), 0.4, 30
+    if name == "config2":
+        return W.config(2), 0.42, 100
+    if name == "config3":
+        return W.config(3), 0.4, 100
+    return W.make_fluid("t", (8, 8, 8), 3.0, seed=33, r_c=1.5, r_cc=1.2, n_species=3), 0.3, 20   # r_c > r_cc, tag 4
+
+
+@pytest.mark.parametrize("name", ["fluid", "config1", "suspension", "config2", "config3", "rc>rcc"])
+def test_neighbor_list_mode_forces_and_trajectory(T, orc, name):
+    w, skin, steps = _list_case(name)
+    sim = T.Simulation.from_workload(w, skin=skin)
+    o = orc.Oracle.from_workload(w)
+    o.compute_forces(0)
+    check_forces(sim, o, label=f"list mode {name} step 0")
+    st = sim.neighbor_list_stats()
+    assert st["rebuilds"] == 1 and st["evaluations"] == 1 and 0 < st["max_entries"] <= st["list_cap"]
+    sim.step(steps)
+    o.step(steps)
+    g, os_ = sim.get_state(), o.get_state()
+    d = min_image_diff(g["pos"], os_["pos"], w.params["box"])
+    assert np.abs(d).max() <= 1e-3 * float(w.params["r_c"]), np.abs(d).max()
+    st = sim.neighbor_list_stats()
+    # the list was reused (fewer binnings than force evaluations) AND rebuilt inside the window
+    assert st["evaluations"] == steps + 1 and 2 <= st["rebuilds"] < st["evaluations"], st
+    print(f"[list] {name}: {st['rebuilds'] - 1} rebuilds in {steps} steps, longest list {st['max_entries']} / {st['list_cap']}")
+    # forces of the state reached through reused lists still agree with the oracle on that state
+    sim.set_state(g["pos"], g["vel"], g["conc"])
+    o.set_state(g["pos"], g["vel"], g["conc"])
+    o.compute_forces(steps)
+    check_forces(sim, o, label=f"list mode {name} step {steps}")
+
+
+def test_neighbor_list_mode_is_deterministic_and_batching_free(T):
+    w = W.small_suspension(seed=3, box=(18, 18, 8), n_rbc=1)
+    a = T.Simulation.from_workload(w, skin=0.35)
+    b = T.Simulation.from_workload(w, skin=0.35)
+    b.set_graph(False)
+    a.step(14)
+    for k in (1, 6, 2, 5):
+        b.step(k)
+    ga, gb = a.get_state(), b.get_state()
+    for k in ("pos", "vel", "conc", "force", "flux"):
+        assert np.array_equal(ga[k], gb[k]), k
+    assert a.neighbor_list_stats()["rebuilds"] == b.neighbor_list_stats()["rebuilds"]
+
+
+def test_neighbor_list_capacity_overflow_is_reported(T):
+    w = W.make_fluid("t", (10, 10, 10), 4.0, seed=5)
+    sim = T.Simulation.from_workload(w, skin=0.4, nlist_cap=64)      # ~130 neighbours within cutoff + skin
+    with pytest.raises(T.TdpdError) as e:
+        sim.get_state()
+    assert e.value.code == -5 and "neighbour list" in str(e.value)
+    with pytest.raises(T.TdpdError):
+        T.Simulation(W.fluid_params((6, 6, 6), 1.0), skin=0.6)      # fewer than 3 cells of edge cutoff + skin
