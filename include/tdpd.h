@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define TDPD_MAX_TYPES 4
-#define TDPD_MAX_SPECIES 4
+#define TDPD_MAX_SPECIES 10 /* the paper benchmarks up to N_spec = 10 */
 
 enum {
   TDPD_OK = 0,

@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "tdpd_oracle.c")
 _LIB = os.path.join(_HERE, "libtdpd_oracle.so")
-T, S = 4, 4
+T, S = 4, 10
 
 
 def build(force: bool = False) -> str:

@@ -22,7 +22,7 @@
 #endif
 
 #define ORC_T 4 /* max particle types   */
-#define ORC_S 4 /* max chemical species */
+#define ORC_S 10 /* max chemical species (PAPER.md:218 benchmarks up to N_spec = 10) */
 
 typedef struct {
   int32_t n_types, n_species;
@@ -158,9 +158,11 @@ int orc_pair_terms(const orc_params *P, int64_t id_i, int64_t id_j, int ti, int 
   if (r2 < 1e-12) return 0;
   if (!(r2 < P->r_cc * P->r_cc) && !(r2 < P->r_c * P->r_c)) return 0;
   double r = sqrt(r2);
-  double g[4], g2[4];
+  /* Gaussians (DESIGN.md R-RNG): tag 0 -> xi = g[0], zeta_0 = g[1], zeta_1 = g[2]; species 2 + 4q .. 5 + 4q take the
+   * four Gaussians of tag 4 + q in order */
+  double g[4], g2[(ORC_S + 1) / 4][4];
   orc_gauss4(id_i, id_j, step, 0u, P->seed, g);
-  if (P->n_species > 2) orc_gauss4(id_i, id_j, step, 4u, P->seed, g2);
+  for (int q = 0; 2 + 4 * q < P->n_species; ++q) orc_gauss4(id_i, id_j, step, 4u + (uint32_t)q, P->seed, g2[q]);
   int kind = 0;
   double inv_sqrt_dt = 1.0 / sqrt(P->dt);
   if (r < P->r_cc) {
@@ -169,7 +171,7 @@ int orc_pair_terms(const orc_params *P, int64_t id_i, int64_t id_j, int ti, int 
     double sgn = id_i < id_j ? 1.0 : -1.0;
     for (int s = 0; s < P->n_species; ++s) {
       double kap = P->kappa[s][ti][tj];
-      double zeta = s == 0 ? g[1] : s == 1 ? g[2] : s == 2 ? g2[0] : g2[1];
+      double zeta = s == 0 ? g[1] : s == 1 ? g[2] : g2[(s - 2) / 4][(s - 2) % 4];
       double wdc = pow(w, P->s_c[s]);
       double wrc = pow(w, 0.5 * P->s_c[s]); /* Eq 10: w_DC = w_RC^2 */
       double csum = Ci[s] + Cj[s];
@@ -231,7 +233,7 @@ static void pair_forces_brute(orc_sim *S) {
 }
 
 /* The oracle's own fp64 cell list: cells of edge >= max(r_c, r_cc), 27-cell stencil.
- * Proven equal to the brute-force search on small boxes (tests/test_oracle_pins.py). */
+ * Proven equal to the brute-force search on small boxes (tests/test_oracle_*.py). */
 static int cell_dims(const orc_params *P, int nc[3]) {
   double rmax = P->r_cc > P->r_c ? P->r_cc : P->r_c;
   for (int a = 0; a < 3; ++a) {
@@ -759,7 +761,8 @@ void orc_neighbor_census(orc_sim *S, int32_t *n_rc, int32_t *n_rcc, uint32_t *xo
       double d[3];
       for (int k = 0; k < 3; ++k) d[k] = min_image(S->x[3 * i + k] - S->x[3 * j + k], P->box[k]);
       double r2 = dot(d, d);
-      if (r2 > 4.0 * P->r_cc * P->r_cc) continue;
+      double rmax = P->r_c > P->r_cc ? P->r_c : P->r_cc;
+      if (r2 > 4.0 * rmax * rmax) continue; /* far beyond both cutoffs: irrelevant to counts and margin */
       double r = sqrt(r2);
       if (r2 >= 1e-12) {
         if (r < P->r_c) { ++a; xa ^= (uint32_t)j; }

@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtdpd.so")
-MAX_TYPES, MAX_SPECIES, N_TIMERS = 4, 4, 7
+MAX_TYPES, MAX_SPECIES, N_TIMERS = 4, 10, 7
 TIMER_NAMES = ("integrate", "sort", "reorder", "pair", "membrane", "closing_kick", "nlist")
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EUNSTABLE = 0, -1, -2, -3, -4, -5
 
@@ -56,7 +56,7 @@ def make_params(p: dict) -> Params:
     P.n_types, P.n_species = int(p["n_types"]), int(p["n_species"])
     for k in ("r_c", "r_cc", "dt", "kBT", "rho"):
         setattr(P, k, float(np.float32(p[k])))
-    for k, n in (("box", 3), ("a", 16), ("gamma", 16), ("s_R", 16), ("kappa", 64), ("s_c", 4), ("m_s", 4),
+    for k, n in (("box", 3), ("a", 16), ("gamma", 16), ("s_R", 16), ("kappa", MAX_SPECIES * 16), ("s_c", MAX_SPECIES), ("m_s", MAX_SPECIES),
                  ("body_force", 3)):
         arr = np.asarray(p[k], dtype=np.float32).ravel()
         if arr.size != n:

@@ -522,7 +522,7 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->F4 = c.take<float4>(n);
   s->Fb = c.take<float4>(n);
   s->Qx = c.take<float>(n * (size_t)std::max(S - 1, 1));
-  s->staging = c.take<float>(n * 4 * 3);  // up to three id-ordered arrays of <= 4 floats per particle
+  s->staging = c.take<float>(n * (size_t)(8 + std::max(S, 4)));  // id-ordered pos [n][4], vel [n][4], conc [n][S]
   s->err_d = c.take<int>(64);
   s->step_d = c.take<uint32_t>(64);
   if (s->nl_skin > 0.0f) {

@@ -22,7 +22,7 @@ from . import mesh as _mesh
 
 BASE_SEED = 20161118
 MAX_TYPES = 4
-MAX_SPECIES = 4
+MAX_SPECIES = 10
 
 BODY_OFF, BODY_UNIFORM, BODY_DOUBLE_POISEUILLE_Z = 0, 1, 2
 

@@ -169,7 +169,7 @@ def test_bond_dissipative_and_random_terms(orc):
     assert np.all(Fr == 0)
     assert np.allclose(np.cross(Fc, e), 0, atol=1e-12)                            # central force
     # Eq 15/16 fluctuation-dissipation: Cov[F^R] = (2 kBT/dt) (gT I + gC e e^T)
-    n = 120_000
+    n = 400_000   # SURVEY §8(c) "Bond random force": >= 4e5 draws
     Ns = rng.standard_normal((n, 9))
     fr = np.array([orc.bond_terms(1.0, 0.01, rp, 0.5, 1.0, d, dv, N)[2] for N in Ns])
     cov = fr.T @ fr / n
