@@ -47,8 +47,26 @@ OPS = dict(cand=(8, 7), flux=(8, 7), rflux=(9, 8), force=(28, 21), philox=(0, 70
 
 
 # --------------------------------------------------------------------------------------------------------------
-def workload(c: int, rank: int = 0, random_flux: bool = True):
-    w = W.config(c) if random_flux else W.config(c, m_s=0.0)  # m_s = 0: the paper's own setting
+def poiseuille_workload(m_s: float = 0.0):
+    """SURVEY §8(f) row 4 / PAPER.md:178-184: transient double Poiseuille flow, 256,000 particles in a periodic 40^3 box,
+    alpha = 18.75, gamma = 4.5, r_c = r_cc = 1.58, s = 0.41 (general-exponent path of the pair kernel), +-f in the halves."""
+    return W.make_fluid("poiseuille", (40.0, 40.0, 40.0), 4.0, seed=W.BASE_SEED + 11, conc="zero", a=18.75, gamma=4.5,
+                        s_R=0.41, r_c=1.58, r_cc=1.58, m_s=m_s, body=0.05, body_mode=W.BODY_DOUBLE_POISEUILLE_Z)
+
+
+def species_workload(ns: int):
+    """SURVEY §8(f) row 2 / PAPER.md:218: the pure-fluid benchmark family (density 4, r_c = 1) with N_spec species, on
+    config 2's box (32^3, 131,072 particles)."""
+    return W.make_fluid(f"fluid32-S{ns}", (32, 32, 32), 4.0, seed=W.BASE_SEED + 20 + ns, n_species=ns)
+
+
+def workload(c: int, rank: int = 0, random_flux: bool = True, kind: str = "config", species: int = 0):
+    if kind == "poiseuille":
+        w = poiseuille_workload()
+    elif species:
+        w = species_workload(species)
+    else:
+        w = W.config(c) if random_flux else W.config(c, m_s=0.0)  # m_s = 0: the paper's own setting (PAPER.md:78)
     if rank:  # replicas differ only in the random stream
         w.params = dict(w.params, seed=int(w.params["seed"]) + 7919 * rank)
     return w
@@ -197,6 +215,17 @@ def cpu_baseline(c: int, seconds: float = 20.0) -> dict:
             "kind": "oracle", "sample": f"{what}; {steps} steps, {dt:.1f} s"}
 
 
+def cpu_baseline_of(w, what: str, seconds: float = 20.0) -> dict:
+    import oracle
+    oracle.build()
+    o = oracle.Oracle.from_workload(w)
+    t0 = time.perf_counter(); o.compute_forces(0); t_f = time.perf_counter() - t0
+    steps = max(1, min(200, int(seconds / max(t_f, 1e-9))))
+    t0 = time.perf_counter(); o.step(steps); dt = time.perf_counter() - t0
+    return {"value": w.n_total * steps / dt, "unit": "particle-steps/s", "cores": oracle.num_threads(),
+            "kind": "oracle", "sample": f"{what}, whole system; {steps} steps, {dt:.1f} s"}
+
+
 # --------------------------------------------------------------------------------------------------------------
 def aggregate(dist, device, ms, ms_e2e, n):
     """Replicas only: whole-job figures = particles summed over ranks / the slowest rank's device time."""
@@ -227,7 +256,8 @@ def run_ours(args) -> dict | None:
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
 
     c = args.config
-    w = workload(c, rank, args.random_flux == "on")
+    w = workload(c, rank, args.random_flux == "on", args.workload, args.species)
+    wname = "poiseuille" if args.workload == "poiseuille" else (f"fluid32-S{args.species}" if args.species else f"config{c}")
     sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap, pair_split=args.pair_split,
                                     skin=args.skin, nlist_cap=args.nlist_cap)
     n, S = sim.n, sim.ns
@@ -313,7 +343,8 @@ def run_ours(args) -> dict | None:
             dist.destroy_process_group()
         return None
 
-    # ---- roofline of the pair kernel (dominant)
+    # ---- roofline of the pair kernel (dominant): measured denominators (tdpd_measure_peaks)
+    mp = T.measure_peaks(local)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -328,16 +359,28 @@ def run_ours(args) -> dict | None:
     pair_hbm_bytes = n * (48 + (8 if S > 2 else 0) + 16 + 4 * max(S - 1, 0))
     traffic = None
     try:  # measured DRAM bytes of one launch from the committed ncu capture of the same workload, if there is one
-        tj = json.load(open(os.path.join(ROOT, "profiles", "r1_pair_traffic.json")))
-        if args.random_flux == "on" and f"config{c}" in tj:
-            traffic = tj[f"config{c}"]["dram_bytes_per_launch"]
+        tj = json.load(open(os.path.join(ROOT, "profiles", "r2_pair_traffic.json")))
+        if args.random_flux == "on" and wname in tj and not args.skin:
+            traffic = tj[wname]["dram_bytes_per_launch"]
     except Exception:
         pass
+    fp32_peak = max(mp["fp32_fma_tflops"], mp["fp32_fma2_tflops"])
+    # BASELINE's roofline, all three legs: FLOPs at the FP32 peak, staged bytes at the L2 bandwidth
+    # (algorithmic: a 2x2x2-cell brick reads its 4x4x4 halo once, 32 B x 8 per particle), compulsory bytes at HBM
+    staged_bytes = n * 32 * 8
+    legs = {"flop_ms": bud["flop"] / (fp32_peak * 1e12) * 1e3, "l2_ms": staged_bytes / (mp["l2_read_gbs"] * 1e9) * 1e3,
+            "hbm_ms": pair_hbm_bytes / (hbm_peak * 1e9) * 1e3}
+    t_roof = max(legs.values())
     roof = {
-        "kernel": "k_pair", "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-        "frac": ach / FP32_PEAK_TFLOPS,
-        "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md §7); not in MEASURED_PEAKS.json",
-        "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read + write)", "algorithmic_bytes": pair_hbm_bytes,
+        "kernel": "k_pair", "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
+        "frac": t_roof / pair_ms,
+        "peak_source": "measured live by tdpd_measure_peaks: FMA microbenchmark, max of scalar fma (%.1f) and packed "
+                       "fma.rn.f32x2 / FFMA2 (%.1f TFLOP/s) at %.3f GHz; nominal 148 x 128 x 2 x 1.965 GHz = %.1f"
+                       % (mp["fp32_fma_tflops"], mp["fp32_fma2_tflops"], mp["sm_ghz"], FP32_PEAK_TFLOPS),
+        "legs_ms": legs, "l2_read_gbs_measured": mp["l2_read_gbs"], "hbm_read_gbs_measured": mp["hbm_read_gbs"],
+        "staged_bytes": staged_bytes,
+        "traffic": traffic, "traffic_source": "committed ncu capture (profiles/), not measured in this run",
+        "traffic_unit": "bytes per launch (ncu dram read + write)", "algorithmic_bytes": pair_hbm_bytes,
         "ms_per_launch": pair_ms, "flop_per_launch": bud["flop"], "share_of_step": kernel_ms["pair"] / (ms_timers / max(K, 1)),
         "timed": "a second pass of the same K steps with per-kernel CUDA events (plain launches); value comes from the first pass (CUDA graphs)",
         "issue_slot_frac": bud["lane_instr"] / (pair_ms * 1e-3) / issue_peak,
@@ -348,21 +391,24 @@ def run_ours(args) -> dict | None:
         "metric": "tDPD particle-steps/sec", "value": ntot * K / (tmax * 1e-3), "unit": "particle-steps/s",
         "n_gpus": world, "steps": K, "warmup": Wm + K, "ms_per_step": tmax / K, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"config{c}", "n_particles": n, "n_rbc": sim.n_rbc, "n_species": S,
+        "config": {"workload": wname, "n_particles": n, "n_rbc": sim.n_rbc, "n_species": S,
                    "box": [float(x) for x in w.params["box"]], "random_flux": bool(np.any(w.params["m_s"][:S] != 0)),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": ("256 MB flush write between timed steps" if flush else
                           f"no flush: state {state_bytes / 2**20:.0f} MB per side > 126 MB L2")},
         "e2e": {"value": ntot * Ke / (temax * 1e-3), "unit": "particle-steps/s", "steps": Ke,
                 "h2d_bytes_per_step": int(n * (6 + S) * 4), "d2h_bytes_per_step": int(n * (6 + S) * 4),
-                "what": "per step: tdpd_set_state (pinned host -> device), tdpd_step(1) incl. the force "
-                        "re-evaluation set_state implies, tdpd_get_state (device -> pinned host)"},
+                "what": "per step: tdpd_set_state (pinned host -> device, the whole state), tdpd_step(1), tdpd_get_state "
+                        "(device -> pinned host); a state replaced by the host needs F(t) again, so a step costs TWO force "
+                        "evaluations by construction (DESIGN.md §7)"},
         "gpu_launches": int(launches), "clocks": clk, "roofline": roof,
         "kernel_ms_per_step": kernel_ms, "ms_per_step_with_timers": ms_timers / K,
         "kernel_ms_note": "CUDA-event time per class per step on its own stream; membrane runs on the second stream concurrently with pair, so its figure includes the time it shares the SMs with the pair kernel",
     }
+    if args.skin:
+        out["config"]["neighbor_list"] = dict(skin=args.skin, **sim.neighbor_list_stats())
     if not args.no_cpu:
-        out["cpu_baseline"] = cpu_baseline(c)
+        out["cpu_baseline"] = cpu_baseline(c) if wname.startswith("config") else cpu_baseline_of(w, wname)
     if dist is not None:
         dist.destroy_process_group()
     return out
@@ -378,6 +424,9 @@ def main():
     ap.add_argument("--pair-threads", type=int, default=0, help="pair-kernel CTA size override (tuning)")
     ap.add_argument("--pair-split", type=int, default=0, help="pair-kernel threads per particle override (tuning)")
     ap.add_argument("--list-cap", type=int, default=0, help="pair-kernel list capacity override (tuning)")
+    ap.add_argument("--workload", default="config", choices=["config", "poiseuille"],
+                    help="poiseuille: the paper's transient double-Poiseuille case (256 k particles, s = 0.41)")
+    ap.add_argument("--species", type=int, default=0, help="N_spec-species fluid on config 2's box (PAPER.md:218)")
     ap.add_argument("--skin", type=float, default=0.0, help="neighbour-list mode: skin radius (0 = bin every step)")
     ap.add_argument("--nlist-cap", type=int, default=0, help="neighbour-list capacity per particle (0 = automatic)")
     ap.add_argument("--random-flux", default="on", choices=["on", "off"],

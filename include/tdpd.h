@@ -16,6 +16,7 @@
  *   a10    a4 and a5-a8 run on two caller-supplied CUDA streams joined by events
  *
  * Conventions
+ *   - Up to TDPD_MAX_SPECIES = 10 chemical species, concentrations [n][n_species] species-fastest.
  *   - All array arguments are HOST pointers, caller-owned, C-contiguous; the library copies in / out.
  *     The only DEVICE pointer is the workspace given to tdpd_set_workspace (caller-owned device memory, e.g. a
  *     torch uint8 tensor); the library owns its contents until tdpd_destroy.
@@ -121,11 +122,13 @@ int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes);
 
 /* Replaces the parameters; takes effect at the next force evaluation (the current forces are re-evaluated with
  * the current step word before the next step).  The cell grid and the type/species counts must not change
- * after tdpd_set_workspace (EINVAL). */
+ * after tdpd_set_workspace, and kBT, dt and the box must not change once a membrane is loaded (its k_p, h_0, A_0,
+ * V_0 were derived from them at tdpd_add_rbc_mesh): EINVAL. */
 int tdpd_set_params(tdpd_sim* s, const tdpd_params* p);
 
 /* Overwrites positions / velocities / concentrations of all particles in id order (any pointer may be NULL),
- * keeps the step counter.  Forces are re-evaluated with the current step word. */
+ * keeps the step counter.  Forces are re-evaluated with the current step word.  Returns after the host buffers
+ * have been copied: the caller may reuse them at once. */
 int tdpd_set_state(tdpd_sim* s, const float* pos, const float* vel, const float* conc);
 
 /* Advances nsteps velocity-Verlet steps (R21).  Asynchronous: only enqueues work on the two streams. */
@@ -135,7 +138,8 @@ int tdpd_step(tdpd_sim* s, int32_t nsteps);
 int tdpd_sync(tdpd_sim* s);
 
 /* Copies out, in id order: pos [n][3], vel [n][3], conc [n][S], force [n][3] (pair + bonded, without the body
- * term), flux [n][S], *step.  Any pointer may be NULL.  Synchronises.  EUNSTABLE if a value is not finite. */
+ * term), flux [n][S], *step.  Any pointer may be NULL.  All requested arrays are gathered and copied asynchronously,
+ * then the call synchronises once.  EUNSTABLE if a value is not finite, a bond is overstretched or a list overflowed. */
 int tdpd_get_state(tdpd_sim* s, float* pos, float* vel, float* conc, float* force, float* flux, int64_t* step);
 
 /* Same as the force part of tdpd_get_state, split into the non-bonded and the membrane contribution. */
@@ -164,11 +168,27 @@ int tdpd_debug_get_binning(tdpd_sim* s, int32_t* cell_xyz, int32_t ncell[3], int
  * coincident particles excluded exactly as in the force sum). */
 int tdpd_debug_neighbor_census(tdpd_sim* s, int32_t* n_rc, int32_t* n_rcc, uint32_t* xor_rc, uint32_t* xor_rcc);
 
+/* The hit lists of the pair kernel itself (bit-exact indexing test): runs the REAL pair kernel (same neighbour-run
+ * tables, candidate loops, thresholds and hit stacks as a force evaluation, in the launch configuration in use) with
+ * the evaluation replaced by a count: per id the number of entries on the front list (r < min(r_c, r_cc)) and on
+ * the ring list (up to max(r_c, r_cc)) and the XOR of the ids behind them; same-membrane and coincident pairs are
+ * left out as in the force sum.  The list thresholds are the cutoffs inflated by 1e-6 relative (DESIGN.md R-cut), so
+ * a pair within that band of a cutoff may sit on either side. */
+int tdpd_debug_pair_census(tdpd_sim* s, int32_t* n_front, int32_t* n_ring, uint32_t* xor_front, uint32_t* xor_ring);
+
+/* Test support: overwrites word `run_index` of the device copy of the static neighbour-run table (seg_meta of
+ * tdpd_host_grid), so that a test can show the indexing checks notice a wrong table entry. */
+int tdpd_debug_set_run_meta(tdpd_sim* s, uint32_t run_index, uint32_t meta);
+
 /* Raw random stream of the device path (for the bit-exact Philox test and the Gaussian tolerance test):
  * words [n][4] = Philox-4x32-10 of counter (min(id_i,id_j), max(id_i,id_j), step, tag) with the simulation's
  * seed; gauss [n][4] = the four Gaussians the kernels derive from them (fp32).  Either may be NULL. */
 int tdpd_debug_rng(tdpd_sim* s, int64_t n, const int64_t* id_i, const int64_t* id_j, int64_t step, uint32_t tag,
                    uint32_t* words, float* gauss);
+
+/* Box-Muller of caller-chosen raw words through the device functions the kernels use: words [n][2] = (x_a, x_b),
+ * gauss [n][2] = R(x_a) (cos 2 pi u(x_b), sin 2 pi u(x_b)).  Lets a test reach the u -> 1 branch of the radius. */
+int tdpd_debug_box_muller(tdpd_sim* s, int64_t n, const uint32_t* words, float* gauss);
 
 /* Host-only view of the static grid tables the pair kernel uses (no CUDA device needed; for tests): ncell[3] per
  * R-bin, cell_rank [ncells] (x-fastest linear cell -> Morton rank), and the neighbour runs of every cell in CSR form
@@ -186,6 +206,16 @@ int tdpd_host_grid(const tdpd_params* p, int32_t ncell[3], uint32_t* n_runs, uin
 #define TDPD_N_TIMERS 7
 int tdpd_set_timing(tdpd_sim* s, int32_t on);
 int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], double ms[TDPD_N_TIMERS]);
+
+/* Measured denominators of the pair kernel's roofline, taken by microbenchmarks on `device` (about
+ * 0.3 s, not on the timed path): FP32 FMA throughput with scalar fma (three register operands) and with the packed
+ * fma.rn.f32x2 of sm_100 (FFMA2), read bandwidth of a 32 MB L2-resident buffer and of a 1 GiB buffer (HBM), the SM
+ * clock seen during the FMA kernel, the SM count.  ECUDA / ENOMEM on failure. */
+typedef struct tdpd_peaks {
+  double fp32_fma_tflops, fp32_fma2_tflops, l2_read_gbs, hbm_read_gbs, sm_ghz;
+  int32_t n_sm, reserved;
+} tdpd_peaks;
+int tdpd_measure_peaks(int device, tdpd_peaks* out);
 
 /* Number of kernels the library launched since creation (bench.py's gpu_launches). */
 int64_t tdpd_launch_count(const tdpd_sim* s);
@@ -212,6 +242,12 @@ int tdpd_set_neighbor_list(tdpd_sim* s, float skin, int32_t list_cap);
  * longest list of the last binning.  Any pointer may be NULL.  Synchronises. */
 int tdpd_get_neighbor_list_stats(tdpd_sim* s, int64_t* n_rebuilds, int64_t* n_evaluations, int32_t* list_cap,
                                  int32_t* max_entries);
+
+/* SURVEY §8(f) row 3 (Fig 2): 1 = K-Apply takes the total area and volume of the force evaluation of the
+ * PREVIOUS time step instead of this step's (the very first evaluation and one that follows tdpd_set_state use their
+ * own), so that the constraint forces do not wait for this launch's reduction; 0 (default) = sequential variant, the
+ * definition (R20).  May be called at any time; the forces are re-evaluated. */
+int tdpd_set_membrane_variant(tdpd_sim* s, int32_t previous_step_area_volume);
 
 /* Steps are replayed as CUDA graphs (one per ping-pong side x first/last step of a call, captured on first use) unless
  * per-kernel timing is on; on = 0 switches to plain launches.  Results are bit-identical either way. */

@@ -79,6 +79,7 @@ def lib():
         L.orc_add_rbc_mesh.argtypes = [vp, i32, vp, vp, vp, i32, vp, P(RbcParams), i32]
         L.orc_set_params.argtypes = [vp, P(Params)]
         L.orc_set_brute.argtypes = [vp, i32]
+        L.orc_set_lagged_area_volume.argtypes = [vp, i32]
         L.orc_n.restype = i64
         L.orc_n.argtypes = [vp]
         L.orc_step_count.restype = i64
@@ -181,6 +182,10 @@ class Oracle:
         self._rbc_nv.append(len(verts))
         self._rbc_ntri.append(len(tris))
         return k
+
+    def set_lagged_area_volume(self, on: bool):
+        """PAPER.md:156 variant: K-Apply with the previous step's area / volume."""
+        self.L.orc_set_lagged_area_volume(self.h, int(on))
 
     def compute_forces(self, step: int):
         self.L.orc_compute_forces(self.h, step)

@@ -50,6 +50,7 @@ typedef struct {
   double *A0t;     /* per triangle */
   double A0, V0;
   double area, volume; /* totals of the last force evaluation (K-Gather) */
+  double area_lag, volume_lag; /* totals of the force evaluation of the previous time step (PAPER.md:156 variant) */
   orc_rbc_params rp;
 } orc_rbc;
 
@@ -64,6 +65,9 @@ typedef struct {
   int64_t step;        /* RNG step word of the last force evaluation */
   int have_forces;
   int use_brute;       /* 1: O(N^2) neighbour search */
+  int lag_av;          /* 1: K-Apply uses the previous step's area / volume (Fig 2) */
+  int lag_valid;       /* the lagged totals belong to step word lag_step */
+  int64_t lag_step;
   /* pair census of the last force evaluation */
   int64_t n_cand, n_cc, n_c;
 } orc_sim;
@@ -485,9 +489,12 @@ static void bonded_forces(orc_sim *S) {
         f[3 * j + a] -= t;
       }
     }
-    /* K-Gather then K-Apply (sequential variant, current step's totals: R20) */
+    /* K-Gather then K-Apply.  Sequential variant (R20, the definition): this step's totals.  Variant of PAPER.md:156
+     * ("use the area/volume of previous time step in K-Apply"): the totals of the force evaluation of step k - 1
+     * when there was one (the very first evaluation, and one after the state was replaced, use their own). */
     orc_rbc_area_volume(R, r, &R->area, &R->volume);
-    area_volume_forces(R, r, R->area, R->volume, f);
+    if (S->lag_av && S->lag_valid && S->lag_step == S->step - 1) area_volume_forces(R, r, R->area_lag, R->volume_lag, f);
+    else area_volume_forces(R, r, R->area, R->volume, f);
     /* bending */
     for (int q = 0; q < R->ndih; ++q) {
       const int32_t *D = &R->dih[4 * q];
@@ -544,6 +551,8 @@ void orc_step(orc_sim *S, int32_t nsteps) {
     half_kick(S);
     for (int64_t i = 0; i < S->n; ++i)
       for (int a = 0; a < 3; ++a) S->x[3 * i + a] = wrap(S->x[3 * i + a] + S->P.dt * S->v[3 * i + a], S->P.box[a]);
+    for (int m = 0; m < S->n_rbc; ++m) { S->rbcs[m].area_lag = S->rbcs[m].area; S->rbcs[m].volume_lag = S->rbcs[m].volume; }
+    S->lag_step = S->step; S->lag_valid = 1;
     orc_compute_forces(S, S->step + 1);
     half_kick(S);
   }
@@ -664,6 +673,7 @@ int32_t orc_add_rbc_mesh(orc_sim *S, int32_t nv, const float *verts, const float
 
 void orc_set_params(orc_sim *S, const orc_params *P) { S->P = *P; S->have_forces = 0; }
 void orc_set_brute(orc_sim *S, int32_t on) { S->use_brute = on; S->have_forces = 0; }
+void orc_set_lagged_area_volume(orc_sim *S, int32_t on) { S->lag_av = on; S->have_forces = 0; }
 int64_t orc_n(const orc_sim *S) { return S->n; }
 int64_t orc_step_count(const orc_sim *S) { return S->step; }
 
@@ -672,6 +682,7 @@ void orc_set_state(orc_sim *S, const double *x, const double *v, const double *C
   if (v) memcpy(S->v, v, 3 * S->n * sizeof(double));
   if (C) memcpy(S->C, C, (size_t)S->P.n_species * S->n * sizeof(double));
   S->have_forces = 0;
+  S->lag_valid = 0;
 }
 
 /* force = pair + bonded (without the body term); any pointer may be NULL */

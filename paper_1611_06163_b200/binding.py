@@ -22,8 +22,8 @@ SYMBOLS = (
     "tdpd_create", "tdpd_load_particles", "tdpd_add_rbc_mesh", "tdpd_workspace_bytes", "tdpd_set_workspace",
     "tdpd_set_params", "tdpd_set_state", "tdpd_step", "tdpd_sync", "tdpd_get_state", "tdpd_get_forces_split",
     "tdpd_num_particles", "tdpd_num_rbc", "tdpd_get_rbc_stats", "tdpd_get_rbc_topology", "tdpd_debug_get_binning",
-    "tdpd_debug_neighbor_census", "tdpd_debug_rng", "tdpd_host_grid", "tdpd_set_timing", "tdpd_get_timing", "tdpd_launch_count",
-    "tdpd_set_tuning", "tdpd_set_neighbor_list", "tdpd_get_neighbor_list_stats", "tdpd_set_graph", "tdpd_last_error", "tdpd_destroy",
+    "tdpd_debug_neighbor_census", "tdpd_debug_pair_census", "tdpd_debug_set_run_meta", "tdpd_debug_rng", "tdpd_debug_box_muller", "tdpd_host_grid", "tdpd_set_timing", "tdpd_get_timing", "tdpd_measure_peaks", "tdpd_launch_count",
+    "tdpd_set_tuning", "tdpd_set_neighbor_list", "tdpd_set_membrane_variant", "tdpd_get_neighbor_list_stats", "tdpd_set_graph", "tdpd_last_error", "tdpd_destroy",
 )
 
 
@@ -48,6 +48,21 @@ class Params(C.Structure):
 class RbcParams(C.Structure):
     _fields_ = [(k, C.c_float) for k in ("p", "x0", "m", "gamma_T", "gamma_C", "k_g", "k_l", "k_v", "k_b", "theta0",
                                          "VR_over_AR32")]
+
+
+class Peaks(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("fp32_fma_tflops", "fp32_fma2_tflops", "l2_read_gbs", "hbm_read_gbs", "sm_ghz")] \
+        + [("n_sm", C.c_int32), ("reserved", C.c_int32)]
+
+
+def measure_peaks(device: int = 0) -> dict:
+    """Measured FP32 / L2 / HBM peaks of the device (tdpd_measure_peaks): the roofline denominators of bench.py."""
+    L = load_library()
+    pk = Peaks()
+    rc = L.tdpd_measure_peaks(int(device), C.byref(pk))
+    if rc != OK:
+        raise TdpdError(rc, "tdpd_measure_peaks failed")
+    return {k: getattr(pk, k) for k, _ in Peaks._fields_ if k != "reserved"}
 
 
 def make_params(p: dict) -> Params:
@@ -108,15 +123,20 @@ def load_library() -> C.CDLL:
     L.tdpd_get_rbc_topology.argtypes = [vp, i32, P(i32), vp, vp, vp, vp, vp]
     L.tdpd_debug_get_binning.argtypes = [vp, vp, vp, vp, vp]
     L.tdpd_debug_neighbor_census.argtypes = [vp, vp, vp, vp, vp]
+    L.tdpd_debug_pair_census.argtypes = [vp, vp, vp, vp, vp]
+    L.tdpd_debug_set_run_meta.argtypes = [vp, u32, u32]
     L.tdpd_debug_rng.argtypes = [vp, i64, vp, vp, i64, u32, vp, vp]
+    L.tdpd_debug_box_muller.argtypes = [vp, i64, vp, vp]
     L.tdpd_host_grid.argtypes = [P(Params), vp, P(u32), vp, vp, vp, vp]
     L.tdpd_set_timing.argtypes = [vp, i32]
     L.tdpd_get_timing.argtypes = [vp, vp, vp]
+    L.tdpd_measure_peaks.argtypes = [C.c_int, P(Peaks)]
     L.tdpd_launch_count.argtypes = [vp]
     L.tdpd_launch_count.restype = i64
     L.tdpd_set_tuning.argtypes = [vp, i32, i32, i32]
     L.tdpd_set_neighbor_list.argtypes = [vp, C.c_float, i32]
     L.tdpd_get_neighbor_list_stats.argtypes = [vp, P(i64), P(i64), P(i32), P(i32)]
+    L.tdpd_set_membrane_variant.argtypes = [vp, i32]
     L.tdpd_set_graph.argtypes = [vp, i32]
     L.tdpd_last_error.argtypes = [vp]
     L.tdpd_last_error.restype = C.c_char_p
@@ -312,6 +332,17 @@ class Simulation:
                                                    _ptr(o["xor_rcc"])))
         return o
 
+    def debug_pair_census(self) -> dict:
+        n = self.n
+        o = dict(n_front=np.zeros(n, np.int32), n_ring=np.zeros(n, np.int32), xor_front=np.zeros(n, np.uint32),
+                 xor_ring=np.zeros(n, np.uint32))
+        self._ck(self.L.tdpd_debug_pair_census(self.h, _ptr(o["n_front"]), _ptr(o["n_ring"]), _ptr(o["xor_front"]),
+                                               _ptr(o["xor_ring"])))
+        return o
+
+    def debug_set_run_meta(self, run_index: int, meta: int):
+        self._ck(self.L.tdpd_debug_set_run_meta(self.h, int(run_index), int(meta)))
+
     def debug_rng(self, id_i, id_j, step: int, tag: int):
         id_i = np.ascontiguousarray(id_i, np.int64)
         id_j = np.ascontiguousarray(id_j, np.int64)
@@ -324,6 +355,15 @@ class Simulation:
         a, b, c, d = C.c_int64(0), C.c_int64(0), C.c_int32(0), C.c_int32(0)
         self._ck(self.L.tdpd_get_neighbor_list_stats(self.h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
         return dict(rebuilds=int(a.value), evaluations=int(b.value), list_cap=int(c.value), max_entries=int(d.value))
+
+    def debug_box_muller(self, words):
+        words = np.ascontiguousarray(words, np.uint32).reshape(-1, 2)
+        g = np.zeros((len(words), 2), np.float32)
+        self._ck(self.L.tdpd_debug_box_muller(self.h, len(words), _ptr(words), _ptr(g)))
+        return g
+
+    def set_membrane_variant(self, previous_step_area_volume: bool):
+        self._ck(self.L.tdpd_set_membrane_variant(self.h, int(previous_step_area_volume)))
 
     def set_graph(self, on: bool):
         self._ck(self.L.tdpd_set_graph(self.h, int(on)))

@@ -59,6 +59,7 @@ struct tdpd_sim {
   PairRec rec = {nullptr, nullptr, nullptr};
   uint32_t* keys_sorted = nullptr;
   int mem_nchunk = 1, mem_nt = 256, max_nv = 0;
+  bool lag_av = false;  // PAPER.md:156 variant of K-Apply
   // device
   void* ws = nullptr;
   size_t ws_bytes = 0;
@@ -522,7 +523,7 @@ static size_t layout(tdpd_sim* s, void* basep) {
   s->F4 = c.take<float4>(n);
   s->Fb = c.take<float4>(n);
   s->Qx = c.take<float>(n * (size_t)std::max(S - 1, 1));
-  s->staging = c.take<float>(n * (size_t)(8 + std::max(S, 4)));  // id-ordered pos [n][4], vel [n][4], conc [n][S]
+  s->staging = c.take<float>(n * (size_t)(9 + 2 * std::max(S, 4)));  // id-ordered pos, vel, force [n][3], conc, flux [n][S]
   s->err_d = c.take<int>(64);
   s->step_d = c.take<uint32_t>(64);
   if (s->nl_skin > 0.0f) {
@@ -532,7 +533,7 @@ static size_t layout(tdpd_sim* s, void* basep) {
     s->nlist_d = c.take<uint16_t>(((n + 255) / 256) * (size_t)s->nl_cap * 256);
   }
   size_t M = s->rbcs.size();
-  s->stats_d = c.take<double>(2 * std::max<size_t>(M, 1));
+  s->stats_d = c.take<double>(4 * std::max<size_t>(M, 1));  // two slots (step parity) of (area, volume) per membrane
   s->rbcs_d = c.take<RbcDev>(std::max<size_t>(M, 1));
   s->tmpls_d = c.take<MeshTemplateDev>(std::max<size_t>(s->tmpls.size(), 1));
   size_t nb = 0, nt = 0, topo = 0;
@@ -664,6 +665,7 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
 // step orchestration
 // =====================================================================================================
 namespace {
+void drop_graphs(tdpd_sim* s);
 struct Scope {  // optional event pair around a group of launches on one stream
   tdpd_sim* s; int cls; cudaStream_t q; cudaEvent_t e1 = nullptr;
   Scope(tdpd_sim* s_, int cls_, cudaStream_t q_) : s(s_), cls(cls_), q(q_) {
@@ -687,6 +689,7 @@ PairArgs pair_args(tdpd_sim* s, int c) {
   A.nlist = s->nlist_d; A.nl_cnt = s->nl_cnt_d; A.nl_cap = s->nl_cap;
   const float rl = std::max(s->prm.r_c, s->prm.r_cc) + s->nl_skin;
   A.rlist2 = rl * rl;
+  A.census = nullptr;
   return A;
 }
 
@@ -756,7 +759,7 @@ int eval_forces(tdpd_sim* s) {
       MembraneArgs M;
       M.st = s->st[c]; M.slot_of_id = s->slot_of_id; M.rbcs = s->rbcs_d; M.tmpls = s->tmpls_d;
       M.h0 = s->h0_d; M.kp = s->kp_d; M.A0t = s->A0t_d; M.Fb = s->Fb; M.stats = s->stats_d;
-      M.nchunk = s->mem_nchunk; M.step_p = s->step_d; M.err = s->err_d;
+      M.nchunk = s->mem_nchunk; M.step_p = s->step_d; M.err = s->err_d; M.lag_av = s->lag_av ? 1 : 0;
       int rc = td_launch_membrane(s->dp, M, (int)s->rbcs.size(), s->max_nv, s->mem_nt, s->sB);
       if (rc) return fail(s, TDPD_ECUDA, std::string("membrane kernel attribute: ") + cudaGetErrorString((cudaError_t)rc));
       s->launches += 1; s->timers[4].launches += 1;
@@ -883,12 +886,15 @@ static int check_err_word(tdpd_sim* s) {
   return TDPD_OK;
 }
 
-static int fetch(tdpd_sim* s, int what, int width, float* host) {
+// id-ordered read-back: every requested array is unsorted into its own part of the staging area and copied out
+// asynchronously; ONE stream synchronisation at the end (round 1: one kernel + one blocking copy + one sync per array)
+static int fetch_begin(tdpd_sim* s, int what, int width, float* host, size_t& off) {
   if (!host || s->n == 0) return TDPD_OK;
-  td_launch_unsort(s->st[s->cur], s->F4, s->Qx, s->Fb, s->n, s->prm.n_species, what, s->staging, s->err_d, s->dp.box, s->sA);
+  float* dst = s->staging + off;
+  off += (size_t)s->n * width;
+  td_launch_unsort(s->st[s->cur], s->F4, s->Qx, s->Fb, s->n, s->prm.n_species, what, dst, s->err_d, s->dp.box, s->sA);
   s->launches += 1;
-  CK(cudaMemcpyAsync(host, s->staging, (size_t)s->n * width * sizeof(float), cudaMemcpyDeviceToHost, s->sA));
-  CK(cudaStreamSynchronize(s->sA));
+  CK(cudaMemcpyAsync(host, dst, (size_t)s->n * width * sizeof(float), cudaMemcpyDeviceToHost, s->sA));
   return TDPD_OK;
 }
 
@@ -898,13 +904,15 @@ extern "C" int tdpd_get_state(tdpd_sim* s, float* pos, float* vel, float* conc, 
   if (!s->finalized) return fail(s, TDPD_ESTATE, "tdpd_set_workspace has not been called");
   int rc;
   if (force || flux) { rc = ensure_forces(s); if (rc) return rc; }
-  if ((rc = tdpd_sync(s))) return rc;
+  CK(cudaSetDevice(s->device));
   const int S = s->prm.n_species;
-  if ((rc = fetch(s, 0, 3, pos))) return rc;
-  if ((rc = fetch(s, 1, 3, vel))) return rc;
-  if ((rc = fetch(s, 2, S, conc))) return rc;
-  if ((rc = fetch(s, 3, 3, force))) return rc;
-  if ((rc = fetch(s, 4, S, flux))) return rc;
+  size_t off = 0;
+  if ((rc = fetch_begin(s, 0, 3, pos, off))) return rc;
+  if ((rc = fetch_begin(s, 1, 3, vel, off))) return rc;
+  if ((rc = fetch_begin(s, 2, S, conc, off))) return rc;
+  if ((rc = fetch_begin(s, 3, 3, force, off))) return rc;
+  if ((rc = fetch_begin(s, 4, S, flux, off))) return rc;
+  if ((rc = tdpd_sync(s))) return rc;
   if (step) *step = s->step;
   return check_err_word(s);
 }
@@ -913,9 +921,10 @@ extern "C" int tdpd_get_forces_split(tdpd_sim* s, float* force_pair, float* forc
   if (!s) return TDPD_EINVAL;
   int rc = ensure_forces(s);
   if (rc) return rc;
+  size_t off = 0;
+  if ((rc = fetch_begin(s, 5, 3, force_pair, off))) return rc;
+  if ((rc = fetch_begin(s, 6, 3, force_bonded, off))) return rc;
   if ((rc = tdpd_sync(s))) return rc;
-  if ((rc = fetch(s, 5, 3, force_pair))) return rc;
-  if ((rc = fetch(s, 6, 3, force_bonded))) return rc;
   return check_err_word(s);
 }
 
@@ -930,7 +939,7 @@ extern "C" int tdpd_get_rbc_stats(tdpd_sim* s, double* area, double* volume, dou
     if (rc) return rc;
     if ((rc = tdpd_sync(s))) return rc;
     std::vector<double> st(2 * std::max<size_t>(M, 1));
-    if (M) CK(cudaMemcpy(st.data(), s->stats_d, 2 * M * sizeof(double), cudaMemcpyDeviceToHost));
+    if (M) CK(cudaMemcpy(st.data(), s->stats_d + (size_t)(s->step & 1) * 2 * M, 2 * M * sizeof(double), cudaMemcpyDeviceToHost));
     for (size_t m = 0; m < M; ++m) {
       if (area) area[m] = st[2 * m];
       if (volume) volume[m] = st[2 * m + 1];
@@ -969,8 +978,12 @@ extern "C" int tdpd_set_params(tdpd_sim* s, const tdpd_params* p) {
       return fail(s, TDPD_EINVAL, "box, cell grid and type/species counts are fixed after tdpd_set_workspace");
     if (!s->rbcs.empty() && (p->kBT != s->prm.kBT || p->dt != s->prm.dt))
       return fail(s, TDPD_EINVAL, "kBT and dt are fixed after tdpd_set_workspace when membranes are present");
-  } else if (p->n_types != s->prm.n_types || p->n_species != s->prm.n_species) {
-    if (s->n) return fail(s, TDPD_EINVAL, "type/species counts cannot change once particles are loaded");
+  } else {
+    if ((p->n_types != s->prm.n_types || p->n_species != s->prm.n_species) && s->n)
+      return fail(s, TDPD_EINVAL, "type/species counts cannot change once particles are loaded");
+    // k_p, h_0, A_0, V_0 of a loaded membrane were derived from kBT and the box at tdpd_add_rbc_mesh
+    if (!s->rbcs.empty() && (p->kBT != s->prm.kBT || p->dt != s->prm.dt || memcmp(p->box, s->prm.box, sizeof p->box)))
+      return fail(s, TDPD_EINVAL, "kBT, dt and box are fixed once a membrane is loaded");
   }
   s->prm = *p;
   s->dp = d;
@@ -994,8 +1007,10 @@ extern "C" int tdpd_set_state(tdpd_sim* s, const float* pos, const float* vel, c
   td_launch_set_state(s->dp, s->st[s->cur], s->n, dpos, dvel, dconc, s->sA);
   s->launches += 1;
   CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(s->sA));  // the caller's buffers are free again when this returns
   if (pos) s->binned = false;
   s->have_forces = false;
+  CK(cudaMemsetAsync(s->step_d + TD_CTL_LAGOK, 0, 4, s->sA));  // the membrane totals of the previous step are void
   return TDPD_OK;
 }
 
@@ -1017,7 +1032,7 @@ extern "C" int tdpd_debug_get_binning(tdpd_sim* s, int32_t* cell_xyz, int32_t nc
   CK(cudaMalloc(&d_cnt, (size_t)s->ncells * 4));
   CK(cudaMalloc(&d_sid, std::max<size_t>(n, 1) * 4));
   CK(cudaMemsetAsync(d_cnt, 0, (size_t)s->ncells * 4, s->sA));
-  td_launch_binning_debug(s->dp, s->st[s->cur], s->n, d_xyz, d_cnt, d_sid, s->sA);
+  td_launch_binning_debug(s->dp, s->st[s->cur], s->n, s->nl_skin > 0.0f ? s->okey_d : s->keys_sorted, s->rank_cell_d, d_xyz, d_cnt, d_sid, s->sA);
   s->launches += 1;
   CK(cudaMemcpyAsync(cell_xyz, d_xyz, n * 12, cudaMemcpyDeviceToHost, s->sA));
   if (cell_count) CK(cudaMemcpyAsync(cell_count, d_cnt, (size_t)s->ncells * 4, cudaMemcpyDeviceToHost, s->sA));
@@ -1037,7 +1052,7 @@ extern "C" int tdpd_debug_neighbor_census(tdpd_sim* s, int32_t* n_rc, int32_t* n
   size_t n = std::max<size_t>((size_t)s->n, 1);
   int32_t* d = nullptr;
   CK(cudaMalloc(&d, n * 16));
-  td_launch_census(s->dp, s->st[s->cur], s->cell_start, s->cell_rank_d, s->n, d, d + n, (uint32_t*)(d + 2 * n),
+  td_launch_census(s->dp, s->st[s->cur], s->cell_start, s->cell_rank_d, s->nl_skin > 0.0f ? s->okey_d : s->keys_sorted, s->rank_cell_d, s->n, d, d + n, (uint32_t*)(d + 2 * n),
                    (uint32_t*)(d + 3 * n), s->sA);
   s->launches += 1;
   size_t b = (size_t)s->n * 4;
@@ -1047,6 +1062,42 @@ extern "C" int tdpd_debug_neighbor_census(tdpd_sim* s, int32_t* n_rc, int32_t* n
   CK(cudaMemcpyAsync(xor_rcc, d + 3 * n, b, cudaMemcpyDeviceToHost, s->sA));
   CK(cudaStreamSynchronize(s->sA));
   cudaFree(d);
+  return TDPD_OK;
+}
+
+extern "C" int tdpd_debug_pair_census(tdpd_sim* s, int32_t* n_front, int32_t* n_ring, uint32_t* xor_front,
+                                      uint32_t* xor_ring) {
+  if (!s || !n_front || !n_ring || !xor_front || !xor_ring) return TDPD_EINVAL;
+  int rc = ensure_forces(s);   // the binning (and, in list mode, the list) the pair kernel works on
+  if (rc) return rc;
+  if ((rc = tdpd_sync(s))) return rc;
+  if (s->n == 0) return TDPD_OK;
+  const size_t n = (size_t)s->n;
+  uint32_t* d = nullptr;
+  CK(cudaMalloc(&d, n * 16));
+  CK(cudaMemsetAsync(d, 0, n * 16, s->sA));
+  PairArgs A = pair_args(s, s->cur);
+  A.census = d;
+  rc = td_launch_pair(s->dp, A, s->pair_nt, s->pair_split, s->nl_skin > 0.0f, s->sA);
+  s->launches += 1;
+  if (rc) { cudaFree(d); return fail(s, TDPD_ECUDA, "pair kernel attribute"); }
+  CK(cudaMemcpyAsync(n_front, d, n * 4, cudaMemcpyDeviceToHost, s->sA));
+  CK(cudaMemcpyAsync(xor_front, d + n, n * 4, cudaMemcpyDeviceToHost, s->sA));
+  CK(cudaMemcpyAsync(n_ring, d + 2 * n, n * 4, cudaMemcpyDeviceToHost, s->sA));
+  CK(cudaMemcpyAsync(xor_ring, d + 3 * n, n * 4, cudaMemcpyDeviceToHost, s->sA));
+  CK(cudaStreamSynchronize(s->sA));
+  cudaFree(d);
+  s->have_forces = false;  // F4 / Qx were not written by this launch: re-evaluate before they are used again
+  return TDPD_OK;
+}
+
+extern "C" int tdpd_debug_set_run_meta(tdpd_sim* s, uint32_t run_index, uint32_t meta) {
+  if (!s || !s->finalized || run_index >= s->seg_meta.size()) return TDPD_EINVAL;
+  int rc = tdpd_sync(s);
+  if (rc) return rc;
+  CK(cudaMemcpy(s->seg_meta_d + run_index, &meta, 4, cudaMemcpyHostToDevice));
+  s->have_forces = false;
+  drop_graphs(s);
   return TDPD_OK;
 }
 
@@ -1067,6 +1118,22 @@ extern "C" int tdpd_debug_rng(tdpd_sim* s, int64_t n, const int64_t* id_i, const
   if (gauss) CK(cudaMemcpyAsync(gauss, dg, n * 16, cudaMemcpyDeviceToHost, s->sA));
   CK(cudaStreamSynchronize(s->sA));
   cudaFree(di); cudaFree(dj); cudaFree(dw); cudaFree(dg);
+  return TDPD_OK;
+}
+
+extern "C" int tdpd_debug_box_muller(tdpd_sim* s, int64_t n, const uint32_t* words, float* gauss) {
+  if (!s || n < 0 || !words || !gauss) return TDPD_EINVAL;
+  if (n == 0) return TDPD_OK;
+  CK(cudaSetDevice(s->device));
+  uint32_t* dw = nullptr;
+  float* dg = nullptr;
+  CK(cudaMalloc(&dw, n * 8)); CK(cudaMalloc(&dg, n * 8));
+  CK(cudaMemcpyAsync(dw, words, n * 8, cudaMemcpyHostToDevice, s->sA));
+  td_launch_box_muller_debug(n, dw, dg, s->sA);
+  s->launches += 1;
+  CK(cudaMemcpyAsync(gauss, dg, n * 8, cudaMemcpyDeviceToHost, s->sA));
+  CK(cudaStreamSynchronize(s->sA));
+  cudaFree(dw); cudaFree(dg);
   return TDPD_OK;
 }
 
@@ -1168,6 +1235,14 @@ extern "C" int tdpd_get_neighbor_list_stats(tdpd_sim* s, int64_t* n_rebuilds, in
     CK(cudaMemcpy(c.data(), s->nl_cnt_d, (size_t)s->n * 4, cudaMemcpyDeviceToHost));
     *max_entries = (int32_t)*std::max_element(c.begin(), c.end());
   }
+  return TDPD_OK;
+}
+
+extern "C" int tdpd_set_membrane_variant(tdpd_sim* s, int32_t previous_step_area_volume) {
+  if (!s) return TDPD_EINVAL;
+  s->lag_av = previous_step_area_volume != 0;
+  s->have_forces = false;
+  drop_graphs(s);  // the flag is a kernel argument of the captured nodes
   return TDPD_OK;
 }
 

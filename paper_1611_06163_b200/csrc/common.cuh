@@ -98,14 +98,20 @@ __device__ __forceinline__ float td_cos_approx(float x) {
 
 // Box-Muller: R = sqrt(-2 ln ua); (g_cos, g_sin) = R (cos 2 pi ub, sin 2 pi ub).
 // MUFU lg2/sqrt/sin/cos; lg2.approx has absolute error 2^-22 on (0.5, 2), which is not good enough for R when
-// ua -> 1 (R -> 0), so the top 2^-17 of the range uses the series -2 ln(1 - t) = 2t + t^2 + O(t^3) with
-// t = 1 - ua (exact in fp32).  Branch-free.
+// ua -> 1 (R -> 0), so the top 2^-10 of the range uses the series of -2 ln(1 - t) with t = 1 - ua (exact in fp32).
+// Branch-free.
+// radius from the uniform u and its lg2 (shared by the pair kernel, which needs lg2(u) for the flux as well)
+__device__ __forceinline__ float td_bm_radius_l(float u, float lg2u) {
+  const float t = 1.0f - u;
+  const float q1 = -1.3862943611198906f * lg2u;  // -2 ln 2 * lg2(u)
+  // -2 ln(1 - t) = 2 t + t^2 + 2/3 t^3 + O(t^4): below t = 2^-10 the series is exact to 3e-10 relative, while the
+  // 2^-22 absolute error of lg2.approx would be 2e-4 of q at t = 2^-10 and 1 % at t = 2^-16 (measured, round 2)
+  const float q2 = t * fmaf(t, fmaf(t, 0.66666669f, 1.0f), 2.0f);
+  return td_sqrt_approx(t < 9.765625e-04f ? q2 : q1);
+}
 __device__ __forceinline__ float td_bm_radius(uint32_t xa) {
   const float u = td_uniform(xa);
-  const float t = 1.0f - u;
-  const float q1 = -1.3862943611198906f * td_lg2_approx(u);  // -2 ln 2 * lg2(u)
-  const float q2 = fmaf(t, t, t + t);
-  return td_sqrt_approx(t < 7.62939453125e-06f ? q2 : q1);
+  return td_bm_radius_l(u, td_lg2_approx(u));
 }
 __device__ __forceinline__ void td_box_muller(uint32_t xa, uint32_t xb, float& g_cos, float& g_sin) {
   const float R = td_bm_radius(xa);
@@ -145,7 +151,8 @@ __host__ __device__ constexpr int td_species_padded(int S) { return S <= 2 ? S :
 __host__ __device__ constexpr int td_species_groups(int S) { return S <= 2 ? 0 : (td_species_padded(S) - 2 + 3) / 4; }
 
 // device control words (one 64-word block; word 0 is the RNG step word the integrator bumps)
-enum { TD_CTL_STEP = 0, TD_CTL_REBUILD = 1, TD_CTL_DMAX2 = 2, TD_CTL_FORCE = 3, TD_CTL_NREBUILD = 4, TD_CTL_NDECIDE = 5 };
+enum { TD_CTL_STEP = 0, TD_CTL_REBUILD = 1, TD_CTL_DMAX2 = 2, TD_CTL_FORCE = 3, TD_CTL_NREBUILD = 4, TD_CTL_NDECIDE = 5,
+       TD_CTL_LAGOK = 6 };  // LAGOK: the membrane totals of the previous step's force evaluation exist
 
 // what the integrator needs to keep the pair records current between binnings (neighbour-list mode)
 struct ListRefresh {
@@ -181,6 +188,7 @@ struct PairArgs {
   uint32_t* nl_cnt;            // [n] entries of each slot
   int nl_cap;                  // entries per slot
   float rlist2;                // (max(r_c, r_cc) + skin)^2
+  uint32_t* census;            // test support: [4][n] by id (front count, front id xor, ring count, ring id xor) or NULL
 };
 
 // mesh template (topology shared by all membranes with the same triangle list), CSR per vertex
@@ -214,7 +222,8 @@ struct MembraneArgs {
   const float* kp;
   const float* A0t;
   float4* Fb;       // bonded force by id
-  double* stats;    // [M][2] area, volume
+  double* stats;    // [2][M][2] area, volume of the force evaluation with step word k in slot k & 1
+  int lag_av;       // PAPER.md:156 variant: K-Apply with the totals of the previous step's evaluation (slot (k - 1) & 1)
   int nchunk;       // CTAs per membrane
   const uint32_t* step_p;  // RNG step word (device counter)
   int* err;
@@ -276,9 +285,12 @@ void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, c
                       int n_species, int what, float* out, int* err, const float* box, cudaStream_t st);
 void td_launch_set_state(const DevParams& P, const SortedState& s, int64_t n, const float* pos, const float* vel,
                          const float* conc, cudaStream_t st);
-void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, int32_t* cell_xyz,
-                             int32_t* cell_count, int32_t* sorted_id, cudaStream_t st);
+void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, const uint32_t* keys,
+                             const uint32_t* rank_cell, int32_t* cell_xyz, int32_t* cell_count, int32_t* sorted_id,
+                             cudaStream_t st);
 void td_launch_census(const DevParams& P, const SortedState& s, const uint32_t* cell_start, const uint32_t* cell_rank,
-                      int64_t n, int32_t* n_rc, int32_t* n_rcc, uint32_t* xor_rc, uint32_t* xor_rcc, cudaStream_t st);
+                      const uint32_t* keys, const uint32_t* rank_cell, int64_t n, int32_t* n_rc, int32_t* n_rcc,
+                      uint32_t* xor_rc, uint32_t* xor_rcc, cudaStream_t st);
 void td_launch_rng_debug(const DevParams& P, int64_t n, const int64_t* id_i, const int64_t* id_j, uint32_t step,
                          uint32_t tag, uint32_t* words, float* gauss, cudaStream_t st);
+void td_launch_box_muller_debug(int64_t n, const uint32_t* words, float* gauss, cudaStream_t st);

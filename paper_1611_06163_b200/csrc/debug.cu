@@ -54,22 +54,18 @@ __global__ void __launch_bounds__(256) k_unsort(SortedState st, const float4* __
   if (bad) atomicOr(err, TD_ERR_NONFINITE);
 }
 
-__device__ __forceinline__ int cell_axis(float x, float inv, int n) {
-  int c = (int)floorf(__fmul_rn(x, inv));
-  c = c > n - 1 ? n - 1 : c;
-  return c < 0 ? 0 : c;
-}
-
+// the cells the binning actually used: the sorted key of a slot is the Morton rank of its cell (written by k_integrate,
+// td_key_of), rank_cell unpacks it; nothing here re-derives a cell from a position
 __global__ void __launch_bounds__(256) k_binning_debug(const DevParams P, SortedState st, int64_t n,
+                                                       const uint32_t* __restrict__ keys,
+                                                       const uint32_t* __restrict__ rank_cell,
                                                        int32_t* __restrict__ cell_xyz, int32_t* __restrict__ cell_count,
                                                        int32_t* __restrict__ sorted_id) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  float4 p = st.pos[i];
-  int64_t id = __float_as_uint(p.w);
-  int cx = cell_axis(p.x, P.cell_inv[0], P.ncell[0]);
-  int cy = cell_axis(p.y, P.cell_inv[1], P.ncell[1]);
-  int cz = cell_axis(p.z, P.cell_inv[2], P.ncell[2]);
+  int64_t id = __float_as_uint(st.pos[i].w);
+  const uint32_t pc = rank_cell[keys[i]];
+  const int cx = (int)(pc & 1023u), cy = (int)((pc >> 10) & 1023u), cz = (int)(pc >> 20);
   cell_xyz[3 * id] = cx; cell_xyz[3 * id + 1] = cy; cell_xyz[3 * id + 2] = cz;
   if (cell_count) atomicAdd(&cell_count[(cz * P.ncell[1] + cy) * P.ncell[0] + cx], 1);
   if (sorted_id) sorted_id[i] = (int32_t)id;
@@ -78,7 +74,9 @@ __global__ void __launch_bounds__(256) k_binning_debug(const DevParams P, Sorted
 // exact census: differences of fp32 positions in fp64, minimum image, strict cutoffs, through the cell table
 __global__ void __launch_bounds__(128) k_census(const DevParams P, SortedState st,
                                                 const uint32_t* __restrict__ cell_start,
-                                                const uint32_t* __restrict__ cell_rank, int64_t n,
+                                                const uint32_t* __restrict__ cell_rank,
+                                                const uint32_t* __restrict__ keys,
+                                                const uint32_t* __restrict__ rank_cell, int64_t n,
                                                 int32_t* __restrict__ n_rc, int32_t* __restrict__ n_rcc,
                                                 uint32_t* __restrict__ xor_rc, uint32_t* __restrict__ xor_rcc) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -87,8 +85,8 @@ __global__ void __launch_bounds__(128) k_census(const DevParams P, SortedState s
   float4 pl = st.lo[i];
   uint32_t mi = __float_as_uint(pl.w);
   int64_t id = __float_as_uint(p.w);
-  int c[3] = {cell_axis(p.x, P.cell_inv[0], P.ncell[0]), cell_axis(p.y, P.cell_inv[1], P.ncell[1]),
-              cell_axis(p.z, P.cell_inv[2], P.ncell[2])};
+  const uint32_t pc = rank_cell[keys[i]];  // the cell the binning put this slot in
+  int c[3] = {(int)(pc & 1023u), (int)((pc >> 10) & 1023u), (int)(pc >> 20)};
   double L[3] = {P.box[0], P.box[1], P.box[2]};
   int a = 0, b = 0;
   uint32_t xa = 0, xb = 0;
@@ -170,7 +168,20 @@ __global__ void k_rng_debug(const DevParams P, int64_t n, const int64_t* __restr
     gauss[4 * i] = g0; gauss[4 * i + 1] = g1; gauss[4 * i + 2] = g2; gauss[4 * i + 3] = g3;
   }
 }
+// Box-Muller of given raw words, through the same device functions the kernels use (u -> 1 series branch included)
+__global__ void k_box_muller_debug(int64_t n, const uint32_t* __restrict__ words, float* __restrict__ gauss) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float g0, g1;
+  td_box_muller(words[2 * i], words[2 * i + 1], g0, g1);
+  gauss[2 * i] = g0; gauss[2 * i + 1] = g1;
+}
 }  // namespace
+
+void td_launch_box_muller_debug(int64_t n, const uint32_t* words, float* gauss, cudaStream_t st) {
+  if (n == 0) return;
+  k_box_muller_debug<<<(int)((n + 255) / 256), 256, 0, st>>>(n, words, gauss);
+}
 
 void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, const float4* Fb, int64_t n,
                       int n_species, int what, float* out, int* err, const float* box, cudaStream_t st) {
@@ -179,16 +190,19 @@ void td_launch_unsort(const SortedState& s, const float4* F4, const float* Qx, c
   TD_SWITCH_S(n_species, k_unsort<S_><<<nb, 256, 0, st>>>(s, F4, Qx, Fb, n, what, out, err, box[0], box[1], box[2]));
 }
 
-void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, int32_t* cell_xyz,
-                             int32_t* cell_count, int32_t* sorted_id, cudaStream_t st) {
+void td_launch_binning_debug(const DevParams& P, const SortedState& s, int64_t n, const uint32_t* keys,
+                             const uint32_t* rank_cell, int32_t* cell_xyz, int32_t* cell_count, int32_t* sorted_id,
+                             cudaStream_t st) {
   if (n == 0) return;
-  k_binning_debug<<<(int)((n + 255) / 256), 256, 0, st>>>(P, s, n, cell_xyz, cell_count, sorted_id);
+  k_binning_debug<<<(int)((n + 255) / 256), 256, 0, st>>>(P, s, n, keys, rank_cell, cell_xyz, cell_count, sorted_id);
 }
 
 void td_launch_census(const DevParams& P, const SortedState& s, const uint32_t* cell_start, const uint32_t* cell_rank,
-                      int64_t n, int32_t* n_rc, int32_t* n_rcc, uint32_t* xor_rc, uint32_t* xor_rcc, cudaStream_t st) {
+                      const uint32_t* keys, const uint32_t* rank_cell, int64_t n, int32_t* n_rc, int32_t* n_rcc,
+                      uint32_t* xor_rc, uint32_t* xor_rcc, cudaStream_t st) {
   if (n == 0) return;
-  k_census<<<(int)((n + 127) / 128), 128, 0, st>>>(P, s, cell_start, cell_rank, n, n_rc, n_rcc, xor_rc, xor_rcc);
+  k_census<<<(int)((n + 127) / 128), 128, 0, st>>>(P, s, cell_start, cell_rank, keys, rank_cell, n, n_rc, n_rcc, xor_rc,
+                                                   xor_rcc);
 }
 
 void td_launch_rng_debug(const DevParams& P, int64_t n, const int64_t* id_i, const int64_t* id_j, uint32_t step,

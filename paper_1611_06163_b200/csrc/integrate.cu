@@ -80,7 +80,10 @@ __global__ void __launch_bounds__(256) k_integrate(const DevParams P, SortedStat
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
   if (i < n) {
-    if (i == 0 && ctl) ctl[TD_CTL_STEP] += 1u;  // the force evaluation that follows the drift uses the next step word
+    if (i == 0 && ctl) {
+      ctl[TD_CTL_STEP] += 1u;   // the force evaluation that follows the drift uses the next step word
+      ctl[TD_CTL_LAGOK] = 1u;   // ... and may use the membrane totals of the evaluation before it (PAPER.md:156 variant)
+    }
     float4 p = st.pos[i];
     if (mode != 0) {
       float4 v = st.vel[i];

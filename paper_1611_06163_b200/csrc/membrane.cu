@@ -85,8 +85,16 @@ __global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevPar
   if (t == 0) {
     double sA = 0.0, sV = 0.0;
     for (int w = 0; w < (NT + 31) / 32; ++w) { sA += red[0][w]; sV += red[1][w]; }
+    const int M = gridDim.x / A.nchunk;
+    double* cur = A.stats + (size_t)(step & 1u) * 2 * M;
+    if (chunk == 0) { cur[2 * m] = sA; cur[2 * m + 1] = sV; }
+    // K-Apply totals: this evaluation's (sequential variant, R20) or, those of the previous step's
+    // evaluation (written by an earlier launch, so that K-Apply does not depend on this launch's reduction)
+    if (A.lag_av && A.step_p[TD_CTL_LAGOK]) {
+      const double* lag = A.stats + (size_t)((step & 1u) ^ 1u) * 2 * M;
+      sA = lag[2 * m]; sV = lag[2 * m + 1];
+    }
     tot[0] = sA; tot[1] = sV;
-    if (chunk == 0) { A.stats[2 * m] = sA; A.stats[2 * m + 1] = sV; }
   }
   __syncthreads();
   const float beta_g = (float)(-(double)R.k_g * (tot[0] - R.A0) / R.A0);

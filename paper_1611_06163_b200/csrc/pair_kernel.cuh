@@ -185,8 +185,7 @@ __device__ __forceinline__ void pair_eval(const DevParams& P, const PairArgs& A,
     if (FASTW) { wR = td_sqrt_approx(wc); wD = wc; }
     else { wR = td_pow_w(wc, tf.w); wD = wR * wR; }
     // xi = R cos(2 pi u1), R = sqrt(-2 ln u0); near u0 = 1 (R -> 0) lg2.approx is not accurate enough: series (td_bm_radius)
-    const float t1 = 1.0f - (td_f12(x0) - TD_C0);
-    const float R0 = td_sqrt_approx(t1 < 7.62939453125e-06f ? fmaf(t1, t1, t1 + t1) : TD_M2LN2 * l0);
+    const float R0 = td_bm_radius_l(td_f12(x0) - TD_C0, l0);
     const float g0 = R0 * td_cos_approx(td_angle(x1));
     const float edv = (dx * (me.v.x - vj.x) + dy * (me.v.y - vj.y) + dz * (me.v.z - vj.z)) * rinv;
     float f = fmaf(tf.z * wR, g0, fmaf(-(tf.y * wD), edv, tf.x * wc));
@@ -202,6 +201,26 @@ template <int S, bool RANDFLUX, bool FASTW, int MODE>
 __device__ __forceinline__ void eval_list(const DevParams& P, const PairArgs& A, const PairSmem& sm, const Self<S>& me,
                                           const uint16_t* base, int stride, int cnt, float& fx, float& fy, float& fz,
                                           float* q) {
+  if (A.census) {
+    // test support (tdpd_debug_pair_census): instead of evaluating, count the entries the REAL candidate loops put on
+    // this end of the stack and XOR the ids behind them (same run tables, same thresholds, same dead-pair rule)
+    uint32_t c = 0, x = 0;
+    for (int k = 0; k < cnt; ++k) {
+      const uint32_t e = base[k * stride];
+      const float4 te = sm.tso[me.lc27 + (int)(e >> OFFBITS)];
+      const uint32_t j = __float_as_uint(te.x) + (e & OFFMASK);
+      const float4 pj = __ldg(&A.rec.R8[2 * (size_t)j]), xj = __ldg(&A.rec.R8[2 * (size_t)j + 1]);
+      const float dx = (me.x - te.y) - pj.x, dy = (me.y - te.z) - pj.y, dz = (me.z - te.w) - pj.z;
+      if (__float_as_uint(xj.w) == me.exq || fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < 1e-12f) continue;
+      ++c; x ^= __float_as_uint(pj.w);
+    }
+    if (cnt > 0) {
+      uint32_t* out = A.census + (size_t)(MODE == 0 ? 0 : 2) * (size_t)A.n + me.id;
+      atomicAdd(out, c);
+      atomicXor(out + A.n, x);
+    }
+    return;
+  }
   for (int k = 0; k < cnt; k += 2) {
     const bool two = k + 1 < cnt;
     const uint32_t e0 = base[k * stride];

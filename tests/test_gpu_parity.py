@@ -55,9 +55,21 @@ def test_philox_words_bit_exact_and_gaussians(T, orc):
         ref = orc.philox_batch(ctr, [seed & 0xFFFFFFFF, seed >> 32])
         assert np.array_equal(words, ref)
         g = orc.gauss_batch(ii, jj, step, tag, seed)
-        assert np.abs(gauss.astype(np.float64) - g).max() < 2e-5
-    # the u -> 1 branch of Box-Muller (R -> 0): force xa into the top 2^-17 by brute search is impractical, so
-    # check the symmetric property instead: xi_ij == xi_ji bit for bit
+        # SURVEY §8(c) proposes 1e-5; measured 1.2e-5: MUFU sin / cos carry ~2e-6 absolute and the radius reaches 5.6
+        assert np.abs(gauss.astype(np.float64) - g).max() < 1.5e-5
+    # the u -> 1 branch of Box-Muller (R -> 0, series instead of lg2.approx): raw words in the top 2^-17 of the range,
+    # around its threshold, at the extremes, against the definition in fp64 (R-RNG)
+    xa = np.concatenate([0xFFFFFFFF - np.arange(0, 70000, 7), np.array([0, 1, 511, 512, 0x7FFFFFFF, 0x80000000]),
+                         (0xFFFFFFFF - 2 ** 15 * 512 + np.arange(-2000, 2000) * 256)]).astype(np.uint32)
+    xb = rng.integers(0, 2 ** 32, len(xa)).astype(np.uint32)
+    gd = sim.debug_box_muller(np.stack([xa, xb], axis=1)).astype(np.float64)
+    ua = ((xa >> 9).astype(np.float64) + 0.5) / 2 ** 23
+    ub = ((xb >> 9).astype(np.float64) + 0.5) / 2 ** 23
+    R = np.sqrt(-2.0 * np.log(ua))
+    ref = np.stack([R * np.cos(2 * np.pi * ub), R * np.sin(2 * np.pi * ub)], axis=1)
+    assert np.abs(gd - ref).max() < 1e-5
+    assert np.abs(gd[:10000] - ref[:10000]).max() < 2e-8               # the series branch: radius <= 6e-3, relative 3e-6
+    # and the symmetric property: xi_ij == xi_ji bit for bit
     w1, g1 = sim.debug_rng(ii[:1000], jj[:1000], 3, 0)
     w2, g2 = sim.debug_rng(jj[:1000], ii[:1000], 3, 0)
     assert np.array_equal(w1, w2) and np.array_equal(g1, g2)
@@ -90,6 +102,65 @@ def test_binning_and_census_bit_exact(T, orc, kind):
     gc = sim.debug_neighbor_census()
     for k in ("n_rc", "n_rcc", "xor_rc", "xor_rcc"):
         assert np.array_equal(gc[k], oc[k]), k
+    check_pair_kernel_lists(sim, oc, w)
+
+
+def check_pair_kernel_lists(sim, oc, w, label=""):
+    """The hit lists of the REAL pair kernel (its neighbour-run tables, candidate loops and stacks) against the oracle's
+    census: the front list holds the pairs within min(r_c, r_cc), front + ring those within max(r_c, r_cc); counts and
+    id checksums must agree bit for bit for every particle none of whose pairs lies inside the 1e-6 inflation band of
+    the list thresholds (such pairs may be on either side)."""
+    pc = sim.debug_pair_census()
+    rc, rcc = float(w.params["r_c"]), float(w.params["r_cc"])
+    inner_is_rc = rc <= rcc
+    n_in = oc["n_rc"] if inner_is_rc else oc["n_rcc"]
+    x_in = oc["xor_rc"] if inner_is_rc else oc["xor_rcc"]
+    n_out = oc["n_rcc"] if inner_is_rc else oc["n_rc"]
+    x_out = oc["xor_rcc"] if inner_is_rc else oc["xor_rc"]
+    clear = oc["margin"] > 4e-6 * max(rc, rcc)
+    assert clear.mean() > 0.99, clear.mean()
+    assert np.array_equal(pc["n_front"][clear], n_in[clear]), label
+    assert np.array_equal(pc["xor_front"][clear], x_in[clear]), label
+    assert np.array_equal((pc["n_front"] + pc["n_ring"])[clear], n_out[clear]), label
+    assert np.array_equal((pc["xor_front"] ^ pc["xor_ring"])[clear], x_out[clear]), label
+    # borderline particles: off by at most the pairs in the band
+    assert np.abs((pc["n_front"] + pc["n_ring"]) - n_out).max() <= 2
+
+
+def test_pair_kernel_lists_in_every_launch_shape(T, orc):
+    """threads per particle 1 / 2 / 16, small stacks (mid-scan drains), neighbour-list mode, r_c > r_cc, a membrane."""
+    w = W.make_fluid("t", (13, 11, 8), 4.0, seed=21)
+    oc = orc.Oracle.from_workload(w).neighbor_census()
+    for kw in (dict(pair_threads=256, pair_split=1), dict(pair_threads=64, list_cap=8, pair_split=1),
+               dict(pair_threads=128, pair_split=2), dict(pair_threads=256, pair_split=16), dict(skin=0.4)):
+        check_pair_kernel_lists(T.Simulation.from_workload(w, **kw), oc, w, label=str(kw))
+    w = W.make_fluid("t", (8, 8, 8), 3.0, seed=33, r_c=1.5, r_cc=1.2)
+    check_pair_kernel_lists(T.Simulation.from_workload(w), orc.Oracle.from_workload(w).neighbor_census(), w)
+    w = W.small_suspension(seed=11, box=(20, 20, 12), n_rbc=1)
+    oc = orc.Oracle.from_workload(w).neighbor_census()
+    check_pair_kernel_lists(T.Simulation.from_workload(w), oc, w)
+    check_pair_kernel_lists(T.Simulation.from_workload(w, skin=0.35), oc, w)
+
+
+def test_pair_kernel_lists_see_a_corrupted_run_table(T, orc):
+    """One wrong entry of the static neighbour-run table (seg_meta: cells in the run | periodic wrap codes) must make
+    the bit-exact check fail: drop one cell from a run, then flip a wrap code."""
+    w = W.make_fluid("t", (10, 10, 10), 4.0, seed=W.BASE_SEED + 1)
+    oc = orc.Oracle.from_workload(w).neighbor_census()
+    grid = T.host_grid(w.params)
+    multi = np.flatnonzero((grid["seg_meta"] & 15) >= 2)
+    for k, new_meta in ((int(multi[len(multi) // 2]), None), (int(multi[3]), "wrap")):
+        sim = T.Simulation.from_workload(w)
+        check_pair_kernel_lists(sim, oc, w)                                   # intact table: passes
+        old = int(grid["seg_meta"][k])
+        sim.debug_set_run_meta(k, old - 1 if new_meta is None else old ^ (3 << 4))
+        with pytest.raises(AssertionError):
+            check_pair_kernel_lists(sim, oc, w)
+        # and the forces of that system are no longer the oracle's
+        o = orc.Oracle.from_workload(w)
+        o.compute_forces(0)
+        with pytest.raises(AssertionError):
+            check_forces(sim, o, label="corrupted table")
 
 
 def test_config1_one_step_forces(T, orc):
@@ -308,32 +379,73 @@ def test_full_size_config_one_step_forces(T, orc, c):
     if w.rbcs:
         gs, ost = sim.rbc_stats(), o.rbc_stats()
         assert np.allclose(gs["area"], ost["area"], rtol=2e-6) and np.allclose(gs["volume"], ost["volume"], rtol=2e-6)
-    # the census of the whole system is bit-exact as well (cells, neighbour counts, neighbour id checksums)
-    if c <= 3:   # (the oracle's census is the slow part: minutes beyond config 3)
-        oc, gc = o.neighbor_census(), sim.debug_neighbor_census()
+    # pair totals of the whole system (directed pairs within r_cc and r_c) from the force evaluation the oracle just did:
+    # bit-exact at every size, and they pin the numerator of bench.py's roofline on the configs it is quoted on
+    tot = o.census_totals()
+    gc = sim.debug_neighbor_census()
+    assert int(gc["n_rcc"].astype(np.int64).sum()) == tot["n_cc"] and int(gc["n_rc"].astype(np.int64).sum()) == tot["n_c"]
+    pc = sim.debug_pair_census()
+    n_all = (pc["n_front"].astype(np.int64) + pc["n_ring"]).sum()
+    assert abs(int(n_all) - tot["n_cc"]) <= max(4, tot["n_cc"] // 200000), (int(n_all), tot["n_cc"])   # 1e-6 band
+    # the census of the whole system is bit-exact per particle as well (cells, neighbour counts, id checksums)
+    if c <= 3:   # (the oracle's O(N^2) census is the slow part: minutes beyond config 3)
+        oc = o.neighbor_census()
         for k in ("n_rc", "n_rcc", "xor_rc", "xor_rcc"):
             assert np.array_equal(gc[k], oc[k]), k
+        check_pair_kernel_lists(sim, oc, w, label=f"config{c}")
 
 
-@pytest.mark.parametrize("c", [2, 3])
+@pytest.mark.parametrize("c", [2, 3, 4, 5])
 def test_full_size_config_100_steps_positions_and_invariants(T, orc, c):
+    import os
+    if c == 5 and not os.environ.get("TDPD_SLOW"):
+        pytest.skip("config 5: 100 oracle steps of 6.9 M particles take ~20 min; run with TDPD_SLOW=1 "
+                    "(last run: profiles/r2_config5_100steps.md)")
     w = W.config(c)
     sim = T.Simulation.from_workload(w)
     o = orc.Oracle.from_workload(w)
     g0 = sim.get_state()
-    sim.step(100)
-    o.step(100)
+    rc = float(w.params["r_c"])
+    sim.step(50)
+    o.step(50)
+    a50 = np.abs(min_image_diff(sim.get_state(forces=False)["pos"], o.get_state(forces=False)["pos"], w.params["box"])).max()
+    sim.step(50)
+    o.step(50)
     g, os_ = sim.get_state(), o.get_state()
     d = min_image_diff(g["pos"], os_["pos"], w.params["box"])
-    assert np.abs(d).max() <= 1e-3 * float(w.params["r_c"]), np.abs(d).max()
+    a = np.abs(d).max(axis=1)
+    q = np.quantile(a, [0.5, 0.9999, 0.99999])
+    print(f"[trajectory] config{c}: max |dx| = {a50:.3e} after 50 steps, {a.max():.3e} after 100 (bar 1e-3 r_c); "
+          f"median {q[0]:.2e}, 99.99 % {q[1]:.2e}, 99.999 % {q[2]:.2e}, beyond the bar: {(a > 1e-3 * rc).sum()} of {len(a)}")
+    assert a50 <= 1e-3 * rc, a50
+    if len(a) < 400_000:
+        assert a.max() <= 1e-3 * rc, a.max()
+    else:
+        # DESIGN.md reading R-traj: the difference of two trajectories grows like exp(5 t) (measured: every quantile of
+        # |dx| grows ~3.5x per 25 steps, identically in configs 2 and 4; tests/test_oracle_dynamics.py shows the same
+        # growth between two runs of the ORACLE whose inputs differ by one fp32 rounding), so the maximum over N
+        # particles is an extreme-value statistic of N: config 4 has 6 particles of 850,632 beyond the bar after 100
+        # steps with the same median and quantiles as config 2.  At these sizes the bar is applied to 99.999 % of the
+        # particles, and the maximum is bounded a decade higher.
+        assert q[2] <= 1e-3 * rc, q
+        assert a.max() <= 1e-2 * rc, a.max()
     # invariants on the GPU side: total concentration conserved; momentum changes only by the body force
     c0, c1 = g0["conc"].astype(np.float64).sum(), g["conc"].astype(np.float64).sum()
     assert abs(c1 - c0) <= 2e-5 * abs(c0)
     p_g, p_o = g["vel"].astype(np.float64).sum(0), os_["vel"].sum(0)
     assert np.abs(p_g - p_o).max() <= 2e-5 * len(d) ** 0.5 * 100
     if w.rbcs:
-        st = sim.rbc_stats()
-        assert np.all(np.abs(st["area"] / st["A0"] - 1) < 5e-3) and np.all(np.abs(st["volume"] / st["V0"] - 1) < 5e-3)
+        # area and volume of every membrane follow the oracle's (the 0.5 % bar of BASELINE.json is for a cell AT REST,
+        # test_rbc_at_rest_holds_area_and_volume; a cell in a driven suspension breathes by what the oracle shows too)
+        st, ot = sim.rbc_stats(), o.rbc_stats()
+        da, dv = np.abs(st["area"] / st["A0"] - 1), np.abs(st["volume"] / st["V0"] - 1)
+        oa, ov = np.abs(ot["area"] / ot["A0"] - 1), np.abs(ot["volume"] / ot["V0"] - 1)
+        print(f"[membranes] config{c} step 100: max |dA/A0| GPU {da.max():.2e} oracle {oa.max():.2e}; "
+              f"max |dV/V0| GPU {dv.max():.2e} oracle {ov.max():.2e}")
+        assert np.allclose(st["area"], ot["area"], rtol=2e-4) and np.allclose(st["volume"], ot["volume"], rtol=2e-4)
+        assert da.max() <= oa.max() + 2e-4 and dv.max() <= ov.max() + 2e-4
+        if len(da) == 1:
+            assert da.max() < 5e-3 and dv.max() < 5e-3
 
 
 def test_pairs_at_the_force_cutoff(T, orc):
@@ -621,3 +733,149 @@ def test_neighbor_list_capacity_overflow_is_reported(T):
     assert e.value.code == -5 and "neighbour list" in str(e.value)
     with pytest.raises(T.TdpdError):
         T.Simulation(W.fluid_params((6, 6, 6), 1.0), skin=0.6)      # fewer than 3 cells of edge cutoff + skin
+
+
+# ---------------------------------------------------------------------------------------------------------
+# many species ("N_spec = 10", layout PAPER.md:146)
+@pytest.mark.parametrize("ns", [5, 7, 10])
+def test_many_species_forces_and_trajectory(T, orc, ns):
+    w = W.make_fluid("t", (16, 16, 16), 4.0, seed=60 + ns, n_species=ns)
+    for kw in (dict(), dict(skin=0.4)):
+        sim = T.Simulation.from_workload(w, **kw)
+        o = orc.Oracle.from_workload(w)
+        o.compute_forces(0)
+        check_forces(sim, o, label=f"{ns} species {kw}")
+        sim.step(20)
+        o.step(20)
+        g, os_ = sim.get_state(), o.get_state()
+        assert np.abs(min_image_diff(g["pos"], os_["pos"], w.params["box"])).max() <= 1e-3
+        assert np.abs(g["conc"] - os_["conc"]).max() <= 1e-4
+        for s in range(ns):   # every species conserved separately
+            assert abs(g["conc"][:, s].astype(np.float64).sum() - w.conc[:, s].astype(np.float64).sum()) <= 1e-5 * len(w.conc)
+
+
+def test_many_species_with_membranes_and_type_dependent_kappa(T, orc):
+    w = W.small_suspension(seed=9, box=(20, 20, 12), n_rbc=1, n_species=6)
+    sim = T.Simulation.from_workload(w)
+    o = orc.Oracle.from_workload(w)
+    o.compute_forces(0)
+    check_forces(sim, o, label="6 species suspension")
+
+
+def test_poiseuille_workload_one_step_forces(T, orc):
+    """SURVEY §8(f) row 4 at production size: 256,000 particles, r_c = r_cc = 1.58, s = 0.41, i.e.
+    the general-exponent (pow) path of the pair kernel, against the oracle."""
+    w = W.make_fluid("poiseuille", (40.0, 40.0, 40.0), 4.0, seed=W.BASE_SEED + 11, conc="zero", a=18.75, gamma=4.5,
+                     s_R=0.41, r_c=1.58, r_cc=1.58, m_s=0.0, body=0.05, body_mode=W.BODY_DOUBLE_POISEUILLE_Z)
+    assert w.n_total == 256000
+    sim = T.Simulation.from_workload(w)
+    o = orc.Oracle.from_workload(w)
+    o.compute_forces(0)
+    check_forces(sim, o, label="poiseuille 256k, s = 0.41")
+    sim.step(10)
+    o.step(10)
+    g, os_ = sim.get_state(), o.get_state()
+    assert np.abs(min_image_diff(g["pos"], os_["pos"], w.params["box"])).max() <= 1e-3 * 1.58
+
+
+# ---------------------------------------------------------------------------------------------------------
+# SURVEY §8(f) row 3: K-Apply with the previous step's area / volume (PAPER.md:156, Fig 2)
+def _soft_cell(seed):
+    """The lagged variant is a delayed feedback: stable only while (omega dt)^2 < 1 for the global area / volume modes.
+    With the P-table constants (k_g = k_v = 20000, dt = 0.01) it blows up within 30 steps IN THE ORACLE AS WELL
+    (k = 5000: same; k = 2000: a slowly growing oscillation, +-20 % in volume after 300 steps on the GPU; k = 20000 at
+    dt = 0.0025: stable with 2-3x the excursions), so the variant is exercised with k_g = k_v = 1000 (R20b)."""
+    w = W.small_suspension(seed=seed, box=(20, 20, 12), n_rbc=1)
+    w.rbc_params = dict(w.rbc_params, k_g=np.float32(1000.0), k_v=np.float32(1000.0))
+    return w
+
+
+def test_previous_step_area_volume_variant_matches_oracle(T, orc):
+    w = _soft_cell(12)
+    for kw in (dict(), dict(skin=0.35)):
+        sim = T.Simulation.from_workload(w, **kw)
+        sim.set_membrane_variant(True)
+        o = orc.Oracle.from_workload(w)
+        o.set_lagged_area_volume(True)
+        o.compute_forces(0)
+        check_forces(sim, o, label="lagged A/V, first evaluation")          # = sequential
+        sim.step(6)
+        o.step(6)
+        g, os_ = sim.get_state(), o.get_state()
+        # no re-synchronisation here (set_state would void the lagged totals): same trajectory to 1e-5, so the stiff
+        # bonded force is compared at 2e-3 of its RMS; the variant itself changes it by far more (checked below)
+        mem = np.flatnonzero(np.abs(os_["force_bonded"]).sum(axis=1) > 0)
+        fb = sim.get_forces_split()[1]
+        err = np.abs(fb[mem] - os_["force_bonded"][mem]).max() / rms(os_["force_bonded"][mem])
+        seq = orc.Oracle.from_workload(w)
+        seq.step(6)
+        gap = np.abs(seq.get_state()["force_bonded"][mem] - os_["force_bonded"][mem]).max() / rms(os_["force_bonded"][mem])
+        print(f"[lagged A/V] GPU vs oracle variant {err:.2e} of RMS; variant vs sequential {gap:.2e} of RMS")
+        assert err < 2e-3 and gap > 10 * err
+        sim.step(44)
+        o.step(44)
+        g, os_ = sim.get_state(), o.get_state()
+        assert np.abs(min_image_diff(g["pos"], os_["pos"], w.params["box"])).max() <= 1e-3
+        gs, ost = sim.rbc_stats(), o.rbc_stats()
+        assert np.allclose(gs["area"], ost["area"], rtol=1e-5) and np.allclose(gs["volume"], ost["volume"], rtol=1e-5)
+
+
+def test_previous_step_variant_is_equivalent_to_the_sequential_one(T):
+    """"the discrepancy ... is insignificant": a cell in driven solvent for 400 steps with both variants
+    (soft constraints, see _soft_cell): area and volume stay together to 1.5 %, the cell's extents (gyration radii) to 3 %,
+    i.e. well within the cell's own breathing (3-6 % at this stiffness)."""
+    w = _soft_cell(13)
+    out = []
+    for lag in (False, True):
+        sim = T.Simulation.from_workload(w)
+        sim.set_membrane_variant(lag)
+        series = []
+        for _ in range(8):
+            sim.step(50)
+            st = sim.rbc_stats()
+            x = sim.get_state(forces=False)["pos"][w.n_solvent:].astype(np.float64)
+            x = x - np.asarray(w.params["box"]) * np.round((x - x[0]) / np.asarray(w.params["box"]))
+            ev = np.sqrt(np.linalg.eigvalsh(np.cov((x - x.mean(0)).T)))
+            series.append([st["area"][0] / st["A0"][0], st["volume"][0] / st["V0"][0], *ev])
+        out.append(np.asarray(series))
+    d = np.abs(out[0] - out[1]) / np.abs(out[0])
+    print(f"[lagged A/V] max relative difference sequential vs previous-step over 400 steps: area {d[:, 0].max():.1e}, "
+          f"volume {d[:, 1].max():.1e}, extents {d[:, 2:].max():.1e}")
+    assert d[:, :2].max() < 1.5e-2 and d[:, 2:].max() < 3e-2     # measured: 3e-3, 8e-3, 1.3e-2
+
+
+def test_rbc_at_rest_holds_area_and_volume(T, orc):
+    """BASELINE north_star / SURVEY §8(c) "RBC at rest": config 3 without the body force: area and volume within 0.5 % of
+    their targets over steps 200..1000 (the oracle's pin of the same statement runs a reduced box for 200 steps)."""
+    w = W.config(3)
+    w.params = dict(w.params, body_force=np.zeros(3, np.float32), body_mode=0)
+    sim = T.Simulation.from_workload(w)
+    sim.step(200)
+    worst = [0.0, 0.0]
+    for _ in range(16):
+        st = sim.rbc_stats()
+        worst[0] = max(worst[0], abs(st["area"][0] / st["A0"][0] - 1))
+        worst[1] = max(worst[1], abs(st["volume"][0] / st["V0"][0] - 1))
+        sim.step(50)
+    print(f"[at rest] config 3, f = 0, steps 200..1000: max |dA/A0| = {worst[0]:.2e}, max |dV/V0| = {worst[1]:.2e}")
+    assert worst[0] < 5e-3 and worst[1] < 5e-3
+
+
+def test_suspension_sample_membrane_excursions_follow_the_oracle(T, orc):
+    """Why the full-length runs of configs 4-5 allow 1 % for the worst of 100 / 1000 cells (test_full_length_run_invariants)
+    while a cell at rest holds 0.5 %: on the 8-cell sample of the config-5 recipe (25.6^3 box, driven flow) the ORACLE
+    shows the same largest area / volume excursions as the GPU over the same 200 steps."""
+    import bench
+    w, _ = bench.sample_workload(5)
+    sim = T.Simulation.from_workload(w)
+    o = orc.Oracle.from_workload(w)
+    ex = np.zeros((2, 2))
+    for _ in range(8):
+        sim.step(25)
+        o.step(25)
+        for k, st in enumerate((sim.rbc_stats(), o.rbc_stats())):
+            ex[k, 0] = max(ex[k, 0], np.abs(st["area"] / st["A0"] - 1).max())
+            ex[k, 1] = max(ex[k, 1], np.abs(st["volume"] / st["V0"] - 1).max())
+    print(f"[membranes] 8-cell sample, 200 steps: max |dA/A0| GPU {ex[0, 0]:.2e} oracle {ex[1, 0]:.2e}; "
+          f"max |dV/V0| GPU {ex[0, 1]:.2e} oracle {ex[1, 1]:.2e}")
+    assert np.abs(ex[0] - ex[1]).max() < 1.5e-3 and ex.max() < 1e-2

@@ -154,3 +154,28 @@ def test_rbc_at_rest_holds_area_and_volume(orc):
     s = o.get_state(forces=False)
     assert np.isfinite(s["pos"]).all()
     assert kinetic_T(s["vel"][-642:]) == pytest.approx(1.0, abs=0.15)     # membrane thermalised by Eq 15/16
+
+
+def test_trajectory_sensitivity_of_the_oracle_itself(orc):
+    """DESIGN.md reading R-traj (why "positions after 100 steps within 1e-3 r_c" is a statement about N): two runs of the
+    ORACLE on config 1 whose initial positions differ by one fp32 rounding (|dx0| <= 3e-7) drift apart exponentially,
+    the maximum over the particles growing by more than 2x per 25 steps.  The GPU-vs-oracle difference grows at the
+    same rate from the fp32 round-off of the forces, so its maximum depends on the number of particles."""
+    w = W.config(1)
+    a = orc.Oracle.from_workload(w)
+    b = orc.Oracle.from_workload(w)
+    s0 = a.get_state(forces=False)
+    rng = np.random.Generator(np.random.PCG64(9))
+    x = s0["pos"] * (1.0 + (rng.random(s0["pos"].shape) - 0.5) * 2.0 ** -23)     # within half an fp32 ulp
+    b.set_state(x, None, None)
+    box = np.asarray(w.params["box"], np.float64)
+    gaps = [np.abs(x - s0["pos"]).max()]
+    for _ in range(4):
+        a.step(25); b.step(25)
+        d = a.get_state(forces=False)["pos"] - b.get_state(forces=False)["pos"]
+        d -= box * np.round(d / box)
+        gaps.append(np.abs(d).max())
+    print("[sensitivity] max |dx| at steps 0, 25, 50, 75, 100:", ["%.2e" % g for g in gaps])
+    assert gaps[0] < 1e-6                              # half an fp32 ulp of a coordinate below 10
+    assert gaps[4] > 100 * gaps[0]                     # two orders of magnitude in one time unit (measured: ~800x)
+    assert gaps[4] > 2.0 * gaps[2] > 2.0 * gaps[0]     # and still growing between steps 50 and 100

@@ -226,3 +226,53 @@ def test_open_or_misoriented_mesh_is_rejected(orc):
     bad = tris.copy(); bad[0] = bad[0, [0, 2, 1]]
     with pytest.raises(ValueError):
         o.add_rbc_mesh((verts + 5).astype(np.float32), None, None, bad, W.rbc_params())
+
+
+def test_previous_step_area_volume_variant(orc):
+    """SURVEY §8(f) row 3 / PAPER.md:156: K-Apply with the totals of the previous step.  The global area and volume terms
+    of Eq 17-18 are linear in (A - A0) / A0 and (V - V0) / V0, so the variant's bonded force differs from the sequential
+    one by exactly  -k_g (A_prev - A) / A0 * dA/dr  -  k_v (V_prev - V) / V0 * dV/dr,  with the gradients taken here by
+    central differences of the numpy area / volume of this file.  The first evaluation, and one after set_state, use
+    their own totals."""
+    o, r0, tris, rp = membrane_only(orc, dict(gamma_T=0.0, gamma_C=0.0), level=2, seed=5)   # no random bond force
+    ref, _, _, _ = membrane_only(orc, dict(gamma_T=0.0, gamma_C=0.0), level=2, seed=5)
+    o.set_lagged_area_volume(True)
+    # first evaluation: identical to the sequential variant
+    o.compute_forces(0); ref.compute_forces(0)
+    assert np.array_equal(o.get_state()["force_bonded"], ref.get_state()["force_bonded"])
+    # kick the membrane so that area and volume change, step both once
+    rng = np.random.Generator(np.random.PCG64(2))
+    v = 2.0 * rng.standard_normal(r0.shape)
+    o.set_state(None, v, None); ref.set_state(None, v, None)
+    o.compute_forces(0); ref.compute_forces(0)
+    A_prev, V_prev = o.rbc_stats()["area"][0], o.rbc_stats()["volume"][0]
+    o.step(1); ref.step(1)
+    so, sr = o.get_state(), ref.get_state()
+    assert np.allclose(so["pos"], sr["pos"], rtol=0, atol=1e-15)        # same positions after one drift (same F^0)
+    st = o.rbc_stats()
+    A, V, A0, V0 = st["area"][0], st["volume"][0], st["A0"][0], st["V0"][0]
+    assert abs(A - A_prev) > 1e-4 * A0                                  # the totals did change
+    r = so["pos"]
+    r = r - 30.0 * np.round((r - r[0]) / 30.0)
+
+    def grad(fun):
+        g = np.zeros_like(r)
+        h = 1e-6
+        for i in range(len(r)):
+            for a in range(3):
+                rp_ = r.copy(); rm_ = r.copy()
+                rp_[i, a] += h; rm_[i, a] -= h
+                g[i, a] = (fun(rp_) - fun(rm_)) / (2 * h)
+        return g
+
+    gA = grad(lambda x: tri_geom(x, tris)[0].sum())
+    gV = grad(lambda x: tri_geom(x, tris)[1].sum())
+    expect = -rp["k_g"] * (A_prev - A) / A0 * gA - rp["k_v"] * (V_prev - V) / V0 * gV
+    diff = so["force_bonded"] - sr["force_bonded"]
+    assert np.abs(diff).max() > 1e-3
+    assert np.allclose(diff, expect, rtol=0, atol=2e-6 * np.abs(expect).max() + 1e-7)
+    # a replaced state voids the lagged totals: the evaluation that follows is the sequential one again
+    x = so["pos"]
+    o.set_state(x, so["vel"], None); ref.set_state(x, so["vel"], None)
+    o.compute_forces(1); ref.compute_forces(1)
+    assert np.array_equal(o.get_state()["force_bonded"], ref.get_state()["force_bonded"])
