@@ -375,8 +375,8 @@ def run_ours(args) -> dict | None:
         "kernel": "k_pair", "bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s",
         "frac": t_roof / pair_ms,
         "peak_source": "measured live by tdpd_measure_peaks: FMA microbenchmark, max of scalar fma (%.1f) and packed "
-                       "fma.rn.f32x2 / FFMA2 (%.1f TFLOP/s) at %.3f GHz; nominal 148 x 128 x 2 x 1.965 GHz = %.1f"
-                       % (mp["fp32_fma_tflops"], mp["fp32_fma2_tflops"], mp["sm_ghz"], FP32_PEAK_TFLOPS),
+                       "fma.rn.f32x2 / FFMA2 (%.1f TFLOP/s); nominal 148 x 128 x 2 x 1.965 GHz = %.1f"
+                       % (mp["fp32_fma_tflops"], mp["fp32_fma2_tflops"], FP32_PEAK_TFLOPS),
         "legs_ms": legs, "l2_read_gbs_measured": mp["l2_read_gbs"], "hbm_read_gbs_measured": mp["hbm_read_gbs"],
         "staged_bytes": staged_bytes,
         "traffic": traffic, "traffic_source": "committed ncu capture (profiles/), not measured in this run",

@@ -210,9 +210,9 @@ int tdpd_get_timing(tdpd_sim* s, int64_t launches[TDPD_N_TIMERS], double ms[TDPD
 /* Measured denominators of the pair kernel's roofline, taken by microbenchmarks on `device` (about
  * 0.3 s, not on the timed path): FP32 FMA throughput with scalar fma (three register operands) and with the packed
  * fma.rn.f32x2 of sm_100 (FFMA2), read bandwidth of a 32 MB L2-resident buffer and of a 1 GiB buffer (HBM), the SM
- * clock seen during the FMA kernel, the SM count.  ECUDA / ENOMEM on failure. */
+ * count.  ECUDA / ENOMEM on failure. */
 typedef struct tdpd_peaks {
-  double fp32_fma_tflops, fp32_fma2_tflops, l2_read_gbs, hbm_read_gbs, sm_ghz;
+  double fp32_fma_tflops, fp32_fma2_tflops, l2_read_gbs, hbm_read_gbs;
   int32_t n_sm, reserved;
 } tdpd_peaks;
 int tdpd_measure_peaks(int device, tdpd_peaks* out);

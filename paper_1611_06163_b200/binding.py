@@ -51,7 +51,7 @@ class RbcParams(C.Structure):
 
 
 class Peaks(C.Structure):
-    _fields_ = [(k, C.c_double) for k in ("fp32_fma_tflops", "fp32_fma2_tflops", "l2_read_gbs", "hbm_read_gbs", "sm_ghz")] \
+    _fields_ = [(k, C.c_double) for k in ("fp32_fma_tflops", "fp32_fma2_tflops", "l2_read_gbs", "hbm_read_gbs")] \
         + [("n_sm", C.c_int32), ("reserved", C.c_int32)]
 
 

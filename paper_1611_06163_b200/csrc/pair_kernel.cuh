@@ -313,7 +313,7 @@ __device__ __forceinline__ void td_push2(uint32_t& pa, uint32_t& pb, float r2, f
 // candidate of each run (adjacent addresses), keep private stacks, and their sums are combined by a fixed xor butterfly.
 // LIST: candidates come from the global neighbour list (SPLIT == 1 only) instead of the 27-cell stencil.
 template <int S, bool RANDFLUX, bool FASTW, int RING, int SPLIT, bool LIST>
-__global__ void __launch_bounds__(256, TD_PAIR_MINB) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
+__global__ void __launch_bounds__(256, (S >= 6 ? 2 : TD_PAIR_MINB)) k_pair(const __grid_constant__ DevParams P, const PairArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int NT = blockDim.x, t = threadIdx.x;
   const int lcap = A.lcap;

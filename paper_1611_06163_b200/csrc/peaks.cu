@@ -6,7 +6,6 @@
 //          the larger of the two is the FP32 peak the roofline uses.
 //   L2:    read-only sweep of a 32 MB buffer (ld.global.cg, 16 B per lane), repeated; the buffer stays L2-resident.
 //   HBM:   the same sweep over 1 GiB.
-//   clock: SM cycles (clock64 span of a CTA) per second of the FFMA kernel.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -15,13 +14,12 @@
 namespace {
 
 template <bool PACKED>
-__global__ void __launch_bounds__(256, 2) k_peak_fma(float* out, uint32_t seed, int iters, unsigned long long* cyc) {
+__global__ void __launch_bounds__(256, 2) k_peak_fma(float* out, uint32_t seed, int iters) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   float a0 = 1.f + t * 1e-9f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f,
         a7 = a0 + 7.f;
   const float b = 1.0000001f + seed * 1e-9f, c = 1e-9f + seed * 1e-12f, b2 = 0.99999f - seed * 1e-9f,
               c2 = 2e-9f + seed * 1e-12f;
-  const unsigned long long t0 = clock64();
 #pragma unroll 1
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
@@ -41,8 +39,6 @@ __global__ void __launch_bounds__(256, 2) k_peak_fma(float* out, uint32_t seed, 
       }
     }
   }
-  const unsigned long long t1 = clock64();
-  if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
   out[t] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
 }
 
@@ -59,13 +55,13 @@ __global__ void __launch_bounds__(256) k_peak_read(const float4* __restrict__ bu
 }
 
 template <bool PACKED>
-bool time_fma(int nsm, float* out, unsigned long long* cyc_d, double* tflops, double* ghz) {
+bool time_fma(int nsm, float* out, double* tflops) {
   const int nblk = 2 * nsm, iters = 40000;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
-  k_peak_fma<PACKED><<<nblk, 256>>>(out, 1, iters / 8, cyc_d);
+  k_peak_fma<PACKED><<<nblk, 256>>>(out, 1, iters / 8);
   cudaEventRecord(e0);
-  k_peak_fma<PACKED><<<nblk, 256>>>(out, 2, iters, cyc_d);
+  k_peak_fma<PACKED><<<nblk, 256>>>(out, 2, iters);
   cudaEventRecord(e1);
   bool ok = cudaDeviceSynchronize() == cudaSuccess;
   float ms = 0.f;
@@ -74,11 +70,6 @@ bool time_fma(int nsm, float* out, unsigned long long* cyc_d, double* tflops, do
   if (!ok || ms <= 0.f) return false;
   const double fma_per_lane = (double)iters * 4 * (PACKED ? 16 : 8);
   *tflops = fma_per_lane * 2.0 * 256.0 * nblk / (ms * 1e-3) / 1e12;
-  unsigned long long c[8] = {0};  // the longest of the first CTAs: a CTA runs for (nearly) the whole launch
-  cudaMemcpy(c, cyc_d, sizeof c, cudaMemcpyDeviceToHost);
-  unsigned long long cm = 0;
-  for (int k = 0; k < 8; ++k) cm = c[k] > cm ? c[k] : cm;
-  *ghz = (double)cm / (ms * 1e-3) / 1e9;
   return true;
 }
 
@@ -110,15 +101,11 @@ extern "C" int tdpd_measure_peaks(int device, tdpd_peaks* out) {
   if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return TDPD_ECUDA;
   const int nsm = prop.multiProcessorCount;
   float* o = nullptr;
-  unsigned long long* cyc = nullptr;
-  if (cudaMalloc(&o, (size_t)nsm * 8 * 256 * 4) != cudaSuccess || cudaMalloc(&cyc, (size_t)nsm * 8 * 8) != cudaSuccess)
-    return TDPD_ENOMEM;
-  double ghz2 = 0.0;
-  bool ok = time_fma<false>(nsm, o, cyc, &out->fp32_fma_tflops, &out->sm_ghz) &&
-            time_fma<true>(nsm, o, cyc, &out->fp32_fma2_tflops, &ghz2) &&
+  if (cudaMalloc(&o, (size_t)nsm * 8 * 256 * 4) != cudaSuccess) return TDPD_ENOMEM;
+  bool ok = time_fma<false>(nsm, o, &out->fp32_fma_tflops) && time_fma<true>(nsm, o, &out->fp32_fma2_tflops) &&
             time_read((size_t)32 << 20, 2000, nsm, o, &out->l2_read_gbs) &&
             time_read((size_t)1 << 30, 50, nsm, o, &out->hbm_read_gbs);
   out->n_sm = nsm;
-  cudaFree(o); cudaFree(cyc);
+  cudaFree(o);
   return ok ? TDPD_OK : TDPD_ECUDA;
 }
