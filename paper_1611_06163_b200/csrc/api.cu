@@ -571,6 +571,12 @@ extern "C" int tdpd_set_workspace(tdpd_sim* s, void* dev_ptr, size_t bytes) {
     if (cudaMalloc(&s->ws, need) != cudaSuccess) return fail(s, TDPD_ENOMEM, "cudaMalloc of the workspace failed");
     s->own_ws = true;
   }
+  {  // list entries address a candidate by an 11-bit offset inside a run of up to 8 (15 at most) cells
+    const double per_run = 8.0 * (double)s->n / std::max<double>(1.0, (double)s->ncells);
+    if (per_run > 1400.0)
+      return fail(s, TDPD_EINVAL, "more than ~175 particles per cell on average: a run of neighbour cells would exceed the 2047 "
+                                  "candidates a list entry can address (use a smaller cutoff-to-density ratio)");
+  }
   s->ws_bytes = need;
   layout(s, s->ws);
   const int64_t n = s->n;

@@ -879,3 +879,20 @@ def test_suspension_sample_membrane_excursions_follow_the_oracle(T, orc):
     print(f"[membranes] 8-cell sample, 200 steps: max |dA/A0| GPU {ex[0, 0]:.2e} oracle {ex[1, 0]:.2e}; "
           f"max |dV/V0| GPU {ex[0, 1]:.2e} oracle {ex[1, 1]:.2e}")
     assert np.abs(ex[0] - ex[1]).max() < 1.5e-3 and ex.max() < 1e-2
+    # kinetic temperature of the suspension after the same 200 steps, by particle class (outer solvent, inner solvent,
+    # membrane vertices): the start-up excess over k_BT = 1 that the full-length runs of configs 4-5 show (1.01-1.03,
+    # test_full_length_run_invariants allows 5 %) is the oracle's as well
+    g, r = sim.get_state(forces=False), o.get_state(forces=False)
+    pos, vel, typ, conc, rid = w.all_particles()
+    kts = []
+    for v in (g["vel"].astype(np.float64), r["vel"]):
+        row = []
+        for t in (0, 1, 2):
+            m = typ == t
+            vv = v[m] - v[m].mean(axis=0)
+            row.append((vv ** 2).sum() / (3 * m.sum() - 3))
+        kts.append(row)
+    kts = np.asarray(kts)
+    print(f"[temperature] 8-cell sample after 200 steps, kT of outer solvent / inner solvent / membrane: GPU "
+          f"{kts[0].round(4).tolist()} oracle {kts[1].round(4).tolist()}")
+    assert np.abs(kts[0] - kts[1]).max() < 5e-3
