@@ -41,9 +41,6 @@
 #ifndef TD_PAIR_MINB
 #define TD_PAIR_MINB 3
 #endif
-#ifndef TD_PAIR_PF
-#define TD_PAIR_PF 0
-#endif
 namespace {
 
 constexpr int MAXLOC = TD_PAIR_MAXLOC;   // cells per table chunk
@@ -402,21 +399,6 @@ __global__ void __launch_bounds__(256, (S >= 6 ? 2 : TD_PAIR_MINB)) k_pair(const
         const float4* __restrict__ src = A.rec.P4 + __float_as_uint(te.x) - ((uint32_t)c << OFFBITS);  // by entry
         const float xs = me.x - te.y, ys = me.y - te.z, zs = me.z - te.w;
         const uint32_t eend = min(ecnt, e + room * SPLIT);
-#if TD_PAIR_PF
-        if (SPLIT == 1) {
-          for (; e + SCAN_UNROLL <= eend; e += SCAN_UNROLL) {
-            // the next group's cache line(s) on their way while this group is tested (no registers held)
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(src + e + SCAN_UNROLL));
-            if (TD_PAIR_PF > 1) asm volatile("prefetch.global.L1 [%0];" ::"l"(src + e + 2 * SCAN_UNROLL - 1));
-#pragma unroll
-            for (int k = 0; k < SCAN_UNROLL; ++k) {
-              const float4 pj = __ldg(&src[e + k]);
-              const float dx = xs - pj.x, dy = ys - pj.y, dz = zs - pj.z;
-              td_push2(pa, pb, fmaf(dz, dz, fmaf(dy, dy, dx * dx)), rin2, rout2, e + k, stride);
-            }
-          }
-        }
-#endif
 #pragma unroll (SPLIT == 1 ? SCAN_UNROLL : 4)
         for (; e < eend; e += SPLIT) {
           const float4 pj = __ldg(&src[e]);
