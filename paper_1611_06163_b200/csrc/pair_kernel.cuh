@@ -41,6 +41,9 @@
 #ifndef TD_PAIR_MINB
 #define TD_PAIR_MINB 3
 #endif
+#ifndef TD_PAIR_F32X2
+#define TD_PAIR_F32X2 1  // packed FADD2 / FMUL2 on the (x, y) pair of a candidate in the stencil scan (-1.3 % kernel time, round 2)
+#endif
 namespace {
 
 constexpr int MAXLOC = TD_PAIR_MAXLOC;   // cells per table chunk
@@ -402,8 +405,19 @@ __global__ void __launch_bounds__(256, (S >= 6 ? 2 : TD_PAIR_MINB)) k_pair(const
 #pragma unroll (SPLIT == 1 ? SCAN_UNROLL : 4)
         for (; e < eend; e += SPLIT) {
           const float4 pj = __ldg(&src[e]);
+#if TD_PAIR_F32X2
+          // x and y of a candidate arrive in an aligned register pair: their difference and square go through the packed
+          // FP32 pipe of sm_100 (FADD2 / FMUL2 in SASS), 5 instead of 6 instructions per distance test
+          float qx, qy;
+          asm("{.reg .b64 s, p, d;\n\tmov.b64 s, {%2, %3};\n\tmov.b64 p, {%4, %5};\n\t"
+              "sub.rn.f32x2 d, s, p;\n\tmul.rn.f32x2 d, d, d;\n\tmov.b64 {%0, %1}, d;\n\t}"
+              : "=f"(qx), "=f"(qy) : "f"(xs), "f"(ys), "f"(pj.x), "f"(pj.y));
+          const float dz = zs - pj.z;
+          const float r2 = fmaf(dz, dz, qx) + qy;
+#else
           const float dx = xs - pj.x, dy = ys - pj.y, dz = zs - pj.z;
           const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+#endif
           td_push2(pa, pb, r2, rin2, rout2, e, stride);
         }
       }
