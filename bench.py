@@ -259,7 +259,7 @@ def run_ours(args) -> dict | None:
     w = workload(c, rank, args.random_flux == "on", args.workload, args.species)
     wname = "poiseuille" if args.workload == "poiseuille" else (f"fluid32-S{args.species}" if args.species else f"config{c}")
     sim = T.Simulation.from_workload(w, device=local, pair_threads=args.pair_threads, list_cap=args.list_cap, pair_split=args.pair_split,
-                                    skin=args.skin, nlist_cap=args.nlist_cap)
+                                    skin=args.skin, nlist_cap=args.nlist_cap, single_stream=args.single_stream)
     n, S = sim.n, sim.ns
     K, Wm = args.steps, max(3, args.warmup)
     state_bytes = n * (16 * 3 + 4 * max(S - 1, 0))
@@ -427,6 +427,8 @@ def main():
     ap.add_argument("--workload", default="config", choices=["config", "poiseuille"],
                     help="poiseuille: the paper's transient double-Poiseuille case (256 k particles, s = 0.41)")
     ap.add_argument("--species", type=int, default=0, help="N_spec-species fluid on config 2's box (PAPER.md:218)")
+    ap.add_argument("--single-stream", action="store_true",
+                    help="membrane kernel on the pair stream instead of its own (shows what the second stream hides)")
     ap.add_argument("--skin", type=float, default=0.0, help="neighbour-list mode: skin radius (0 = bin every step)")
     ap.add_argument("--nlist-cap", type=int, default=0, help="neighbour-list capacity per particle (0 = automatic)")
     ap.add_argument("--random-flux", default="on", choices=["on", "off"],

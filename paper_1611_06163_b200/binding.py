@@ -176,7 +176,8 @@ class Simulation:
     """One tDPD + RBC simulation on one GPU.  Methods mirror the C ABI one to one."""
 
     def __init__(self, params: dict, device: int = 0, pair_threads: int = 0, list_cap: int = 0,
-                 pair_split: int = 0, skin: float = 0.0, nlist_cap: int = 0):
+                 pair_split: int = 0, skin: float = 0.0, nlist_cap: int = 0,
+                 single_stream: bool = False):
         import torch
 
         self.L = load_library()
@@ -189,7 +190,8 @@ class Simulation:
         self._P = make_params(params)
         with torch.cuda.device(self.device):
             self.stream_pair = torch.cuda.Stream(device=self.device)
-            self.stream_bonded = torch.cuda.Stream(device=self.device, priority=-1)  # membrane kernel first
+            # membrane kernel on its own, higher-priority stream (single_stream: on the pair stream, to measure the overlap)
+            self.stream_bonded = self.stream_pair if single_stream else torch.cuda.Stream(device=self.device, priority=-1)
         h = C.c_void_p()
         rc = self.L.tdpd_create(C.byref(self._P), self.device, C.c_void_p(self.stream_pair.cuda_stream),
                                 C.c_void_p(self.stream_bonded.cuda_stream), C.byref(h))
