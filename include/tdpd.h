@@ -75,6 +75,11 @@ typedef struct tdpd_params {
   uint64_t seed;
   int32_t exclude_same_cell_membrane_pairs;     /* R16 */
   int32_t reserved;
+  /* Source term of Eq 7 (PAPER.md:63, :78 "external concentration source", :272 "reacts with the solvent and
+   * dissipates"; the paper gives no form: DESIGN.md reading R-QS): Q^S_i = source[s][type_i] - decay[s][type_i] C_i^s,
+   * added to the flux of every force evaluation.  All zero = no source. */
+  float source[TDPD_MAX_SPECIES][TDPD_MAX_TYPES];
+  float decay[TDPD_MAX_SPECIES][TDPD_MAX_TYPES];
 } tdpd_params;
 
 /* Membrane model parameters (values are inputs, R11). */

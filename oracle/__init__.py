@@ -31,7 +31,8 @@ class Params(C.Structure):
                 ("rho", C.c_double), ("a", C.c_double * (T * T)), ("gamma", C.c_double * (T * T)),
                 ("s_R", C.c_double * (T * T)), ("kappa", C.c_double * (S * T * T)), ("s_c", C.c_double * S),
                 ("m_s", C.c_double * S), ("body_force", C.c_double * 3), ("body_mode", C.c_int32),
-                ("seed", C.c_uint64), ("exclude_same_cell_membrane_pairs", C.c_int32)]
+                ("seed", C.c_uint64), ("exclude_same_cell_membrane_pairs", C.c_int32),
+                ("source", C.c_double * (S * T)), ("decay", C.c_double * (S * T))]
 
 
 class RbcParams(C.Structure):
@@ -50,6 +51,11 @@ def make_params(p: dict) -> Params:
         arr = np.asarray(p[k], dtype=np.float32).astype(np.float64).ravel()
         assert arr.size == n, k
         getattr(P, k)[:] = arr.tolist()
+    for k in ("source", "decay"):
+        if k in p:
+            arr = np.asarray(p[k], dtype=np.float32).astype(np.float64).ravel()
+            assert arr.size == S * T, k
+            getattr(P, k)[:] = arr.tolist()
     P.body_mode = int(p["body_mode"])
     P.seed = int(p["seed"])
     P.exclude_same_cell_membrane_pairs = int(p["exclude_same_cell_membrane_pairs"])

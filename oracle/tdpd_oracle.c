@@ -34,6 +34,8 @@ typedef struct {
   int32_t body_mode; /* 0 off, 1 uniform, 2 double Poiseuille in z */
   uint64_t seed;
   int32_t exclude_same_cell_membrane_pairs;
+  /* Q^S of Eq 7 (reading R-QS): Q^S_i = source[s][type_i] - decay[s][type_i] C_i^s */
+  double source[ORC_S][ORC_T], decay[ORC_S][ORC_T];
 } orc_params;
 
 typedef struct {
@@ -527,6 +529,10 @@ void orc_compute_forces(orc_sim *S, int64_t step) {
   memset(S->Fb, 0, 3 * S->n * sizeof(double));
   memset(S->Q, 0, (size_t)S->P.n_species * S->n * sizeof(double));
   if (S->use_brute) pair_forces_brute(S); else pair_forces_cells(S);
+  /* source term Q^S_i of Eq 7: external source and first-order reaction, by species and particle type */
+  for (int64_t i = 0; i < S->n; ++i)
+    for (int s = 0; s < S->P.n_species; ++s)
+      S->Q[(size_t)S->P.n_species * i + s] += S->P.source[s][S->type[i]] - S->P.decay[s][S->type[i]] * S->C[(size_t)S->P.n_species * i + s];
   bonded_forces(S);
   body_forces(S);
   S->have_forces = 1;

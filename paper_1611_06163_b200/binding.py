@@ -42,7 +42,8 @@ class Params(C.Structure):
                 ("kappa", C.c_float * (MAX_SPECIES * MAX_TYPES * MAX_TYPES)),
                 ("s_c", C.c_float * MAX_SPECIES), ("m_s", C.c_float * MAX_SPECIES),
                 ("body_force", C.c_float * 3), ("body_mode", C.c_int32), ("seed", C.c_uint64),
-                ("exclude_same_cell_membrane_pairs", C.c_int32), ("reserved", C.c_int32)]
+                ("exclude_same_cell_membrane_pairs", C.c_int32), ("reserved", C.c_int32),
+                ("source", C.c_float * (MAX_SPECIES * MAX_TYPES)), ("decay", C.c_float * (MAX_SPECIES * MAX_TYPES))]
 
 
 class RbcParams(C.Structure):
@@ -77,6 +78,12 @@ def make_params(p: dict) -> Params:
         if arr.size != n:
             raise ValueError(f"parameter {k}: expected {n} values, got {arr.size}")
         getattr(P, k)[:] = arr.tolist()
+    for k in ("source", "decay"):   # optional: Q^S (zero when absent)
+        if k in p:
+            arr = np.asarray(p[k], dtype=np.float32).ravel()
+            if arr.size != MAX_SPECIES * MAX_TYPES:
+                raise ValueError(f"parameter {k}: expected {MAX_SPECIES * MAX_TYPES} values, got {arr.size}")
+            getattr(P, k)[:] = arr.tolist()
     P.body_mode = int(p["body_mode"])
     P.seed = int(p["seed"])
     P.exclude_same_cell_membrane_pairs = int(p["exclude_same_cell_membrane_pairs"])

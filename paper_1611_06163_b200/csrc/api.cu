@@ -178,6 +178,11 @@ void derive_params(const tdpd_params& p, DevParams& d, float skin = 0.0f) {
     if (p.s_c[sp] != 2.0f) fast = false;
     if (p.m_s[sp] != 0.0f) rnd = true;
   }
+  for (int sp = 0; sp < p.n_species; ++sp)
+    for (int t = 0; t < p.n_types; ++t) {
+      d.src[sp][t] = p.source[sp][t]; d.dec[sp][t] = p.decay[sp][t];
+      if (p.source[sp][t] != 0.0f || p.decay[sp][t] != 0.0f) d.has_source = 1;
+    }
   d.body_mode = p.body_mode;
   uint32_t k0 = (uint32_t)(p.seed & 0xffffffffu), k1 = (uint32_t)(p.seed >> 32);
   for (int r = 0; r < 10; ++r) {

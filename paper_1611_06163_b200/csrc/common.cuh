@@ -36,6 +36,8 @@ struct DevParams {
   int excl_same;
   int fast_w;     // every s_R == 0.5 and every s_c == 2: weights need no pow
   int rand_flux;  // some m_s != 0
+  int has_source; // some source / decay rate != 0
+  float src[TD_S][TD_T], dec[TD_S][TD_T];  // Q^S_i = src[s][type] - dec[s][type] C_i^s  (Eq 7, reading R-QS)
 };
 
 // meta word of a particle: bits 0-1 type, bits 2-31 membrane id + 1 (0 = free particle)

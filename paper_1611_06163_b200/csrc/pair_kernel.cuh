@@ -463,6 +463,13 @@ __global__ void __launch_bounds__(256, (S >= 6 ? 2 : TD_PAIR_MINB)) k_pair(const
       }
     }
     if (mine && sub == 0) {
+      if (P.has_source) {  // Q^S_i of Eq 7: external source and first-order reaction by species and type
+        td_pair_load_self<S>(P, A, i, me);
+        const int ty = me.t4 / TD_T;
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+          if (s < P.n_species) q[s] += P.src[s][ty] - P.dec[s][ty] * me.c[s];
+      }
       A.F4[i] = make_float4(fx, fy, fz, q[0]);
 #pragma unroll
       for (int s = 1; s < S; ++s)

@@ -38,7 +38,7 @@ def _f32(x):
 
 def fluid_params(box, rho, n_species=1, a=None, gamma=4.5, kBT=1.0, s_R=0.5, kappa=10.0, kappa_m=1.0,
                  s_c=2.0, m_s=0.01, r_c=1.0, r_cc=1.58, dt=0.01, body=0.0, body_mode=BODY_OFF, seed=1,
-                 n_types=1):
+                 n_types=1, source=0.0, decay=0.0):
     """Parameter dict mirroring `tdpd_params` (include/tdpd.h).  Types: 0 outer solvent, 1 inner
     solvent, 2 membrane: kappa_00 = kappa_11 = kappa, kappa_01 = 0,
     kappa_x2 = kappa_m."""
@@ -56,6 +56,9 @@ def fluid_params(box, rho, n_species=1, a=None, gamma=4.5, kBT=1.0, s_R=0.5, kap
         if n_types >= 3:
             K[s, 2, :n_types] = kappa_m
             K[s, :n_types, 2] = kappa_m
+    SRC = np.zeros((S, T)); DEC = np.zeros((S, T))     # Q^S: the same rate for every species, per type if a sequence
+    SRC[:n_species, :n_types] = np.asarray(source, dtype=np.float64)
+    DEC[:n_species, :n_types] = np.asarray(decay, dtype=np.float64)
     sc = np.zeros(S); ms = np.zeros(S)
     sc[:n_species] = s_c
     ms[:n_species] = m_s
@@ -64,7 +67,7 @@ def fluid_params(box, rho, n_species=1, a=None, gamma=4.5, kBT=1.0, s_R=0.5, kap
         r_cc=np.float32(r_cc), dt=np.float32(dt), kBT=np.float32(kBT), rho=np.float32(rho),
         a=_f32(A), gamma=_f32(G), s_R=_f32(SR), kappa=_f32(K), s_c=_f32(sc), m_s=_f32(ms),
         body_force=_f32([body, 0.0, 0.0]), body_mode=int(body_mode), seed=int(seed),
-        exclude_same_cell_membrane_pairs=1,
+        exclude_same_cell_membrane_pairs=1, source=_f32(SRC), decay=_f32(DEC),
     )
 
 

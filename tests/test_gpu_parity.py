@@ -896,3 +896,22 @@ def test_suspension_sample_membrane_excursions_follow_the_oracle(T, orc):
     print(f"[temperature] 8-cell sample after 200 steps, kT of outer solvent / inner solvent / membrane: GPU "
           f"{kts[0].round(4).tolist()} oracle {kts[1].round(4).tolist()}")
     assert np.abs(kts[0] - kts[1]).max() < 5e-3
+
+
+def test_source_term_matches_oracle(T, orc):
+    """Q^S of Eq 7 (reading R-QS): source and first-order decay by species and type, in the flux of every
+    force evaluation and through 50 steps, scan and list mode, with membranes as the sources."""
+    w = W.small_suspension(seed=14, box=(20, 20, 12), n_rbc=1, n_species=2, source=[0.0, 0.0, 0.6], decay=[0.4, 0.0, 0.0])
+    for kw in (dict(), dict(skin=0.35)):
+        sim = T.Simulation.from_workload(w, **kw)
+        o = orc.Oracle.from_workload(w)
+        o.compute_forces(0)
+        check_forces(sim, o, label=f"source term {kw}")
+        sim.step(50)
+        o.step(50)
+        g, os_ = sim.get_state(), o.get_state()
+        assert np.abs(g["conc"] - os_["conc"]).max() <= 2e-4
+        assert np.abs(min_image_diff(g["pos"], os_["pos"], w.params["box"])).max() <= 1e-3
+    # the totals moved by what the source put in and the decay took out (no longer conserved)
+    c0 = w.all_particles()[3].astype(np.float64).sum(axis=0)
+    assert np.all(np.abs(g["conc"].astype(np.float64).sum(axis=0) - c0) > 1.0)

@@ -179,3 +179,34 @@ def test_trajectory_sensitivity_of_the_oracle_itself(orc):
     assert gaps[0] < 1e-6                              # half an fp32 ulp of a coordinate below 10
     assert gaps[4] > 100 * gaps[0]                     # two orders of magnitude in one time unit (measured: ~800x)
     assert gaps[4] > 2.0 * gaps[2] > 2.0 * gaps[0]     # and still growing between steps 50 and 100
+
+
+def test_source_term_first_order_kinetics(orc):
+    """Q^S of Eq 7 (reading R-QS): Q^S_i = source - decay C_i by species and type.  With a
+    uniform concentration the Fickian flux vanishes (m_s = 0: no random flux), so every particle follows
+    dC/dt = q - k C:  C(t) = q/k + (C_0 - q/k) exp(-k t), whatever the particles do."""
+    q, k, C0 = 0.3, 0.8, 1.5
+    w = W.make_fluid("t", (6, 6, 6), 3.0, seed=4, m_s=0.0, source=q, decay=k)
+    w.conc[:] = C0
+    o = orc.Oracle.from_workload(w)
+    o.step(100)
+    C = o.get_state(forces=False)["conc"][:, 0]
+    exact = q / k + (C0 - q / k) * np.exp(-k * 1.0)
+    assert np.ptp(C) < 1e-12                                   # uniform stays uniform
+    assert C.mean() == pytest.approx(exact, rel=3e-3)          # Q is evaluated with the half-step C (R21): first order in dt
+    # halving the time step halves the error
+    e = []
+    for dt, n in ((0.02, 50), (0.01, 100)):
+        w2 = W.make_fluid("t", (6, 6, 6), 3.0, seed=4, m_s=0.0, source=q, decay=k, dt=dt)
+        w2.conc[:] = C0
+        o2 = orc.Oracle.from_workload(w2)
+        o2.step(n)
+        e.append(abs(o2.get_state(forces=False)["conc"][:, 0].mean() - exact))
+    assert 1.7 < e[0] / e[1] < 2.4
+    # by type: only type-1 particles decay; and the flux reported at a force evaluation contains Q^S
+    p = W.fluid_params((6, 6, 6), 3.0, n_types=2, m_s=0.0, kappa=0.0, decay=[0.0, 2.0], seed=4)
+    o3 = orc.Oracle(p)
+    pos = np.array([[1, 1, 1], [4, 4, 4]], np.float32)
+    o3.load_particles(pos, np.zeros((2, 3), np.float32), np.array([0, 1], np.int32), np.array([[0.5], [0.5]], np.float32))
+    o3.compute_forces(0)
+    assert np.allclose(o3.get_state()["flux"][:, 0], [0.0, -1.0], atol=1e-7)
