@@ -9,9 +9,11 @@
  * Every function cites the passage it follows.  Readings of silent / garbled passages are the
  * ones listed in DESIGN.md §"Readings" (R1..), which follow SURVEY.md §8(c) A1..A26.
  *
- * Parity status: the cross-membrane coefficient reading (R15: kappa_ij by type pair) and the
- * RBC parameter values are inputs with no independent pin — "parity unpinned" beyond
- * conservation.  Everything else is pinned by tests/test_oracle_*.py.
+ * Parity status: the cross-membrane coefficient reading (R15: kappa_ij by type pair), the form
+ * of the source term Q^S (R-QS: zeroth-order source + first-order decay by species and type) and
+ * the RBC parameter values are inputs / readings with no independent pin — "parity unpinned"
+ * beyond conservation and the closed form of dC/dt = q - kC.  Everything else is
+ * pinned by tests/test_oracle_*.py.
  */
 #include <math.h>
 #include <stdint.h>
