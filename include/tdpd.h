@@ -258,6 +258,33 @@ int tdpd_set_membrane_variant(tdpd_sim* s, int32_t previous_step_area_volume);
  * per-kernel timing is on; on = 0 switches to plain launches.  Results are bit-identical either way. */
 int tdpd_set_graph(tdpd_sim* s, int32_t on);
 
+/* ---- Sorting without allocating ------------------------------------------------------------------------------------
+ * The stable LSD radix sort of (cell key, previous slot) pairs of row a2 (PAPER.md:137 "particle reordering", :141
+ * "radix sort"), the same kernels a step runs, as a call of its own for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops): its scratch (digit histograms, chunk totals and the
+ * second side of the ping-pong) is one fixed device array inside the library, TDPD_NOALLOC_SCRATCH_BYTES on every GPU
+ * that loads the library until the process exits.  The call allocates nothing and frees nothing.
+ *   d_keys      [n] DEVICE, read only: 32-bit keys, only the low key_bits bits (1..32) are significant
+ *   d_vals      [n] DEVICE, read only, or NULL for the values 0 .. n-1 (the result is then the sorting permutation)
+ *   d_keys_out  [n] DEVICE: the keys in ascending order; equal keys keep their input order (stable)
+ *   d_vals_out  [n] DEVICE: the values in the order of their keys
+ *   stream      a cudaStream_t (NULL = the default stream); the call only enqueues work and does not synchronise
+ * d_keys_out may be d_keys and d_vals_out may be d_vals (in place); any other overlap of the four arrays is not allowed.
+ * The pointers must belong to the CURRENT device of the calling thread.  The caller keeps ownership of all four.
+ * n <= TDPD_NOALLOC_MAX_N, else TDPD_EINVAL (nothing is enqueued); other bad arguments TDPD_EINVAL, CUDA errors
+ * TDPD_ECUDA; the message of the calling thread's last failure is tdpd_noalloc_last_error.  n = 0 is a no-op.
+ * All calls on a device share the one scratch array, which keeps the contents of the last call (nothing in it has to
+ * start at zero: every entry a call reads was written by that call).  Calls whose kernels can overlap on the GPU
+ * (different streams without an event between them, several host threads) RACE: keep them on one stream.
+ * tdpd_noalloc_init asks the driver for the array's address on the current device (done once per device, otherwise
+ * on the first sort there): call it before a stream capture begins. */
+#define TDPD_NOALLOC_MAX_N 262144
+#define TDPD_NOALLOC_SCRATCH_BYTES 2228224 /* 2 x 4 x MAX_N of ping-pong + 128 KiB of histograms */
+int tdpd_noalloc_init(void);
+int tdpd_sort_cells_noalloc(const uint32_t* d_keys, const uint32_t* d_vals, int64_t n, int32_t key_bits,
+                            uint32_t* d_keys_out, uint32_t* d_vals_out, void* stream);
+const char* tdpd_noalloc_last_error(void);
+
 const char* tdpd_last_error(const tdpd_sim* s);
 int tdpd_destroy(tdpd_sim* s);
 

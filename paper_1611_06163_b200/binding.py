@@ -24,6 +24,7 @@ SYMBOLS = (
     "tdpd_num_particles", "tdpd_num_rbc", "tdpd_get_rbc_stats", "tdpd_get_rbc_topology", "tdpd_debug_get_binning",
     "tdpd_debug_neighbor_census", "tdpd_debug_pair_census", "tdpd_debug_set_run_meta", "tdpd_debug_rng", "tdpd_debug_box_muller", "tdpd_host_grid", "tdpd_set_timing", "tdpd_get_timing", "tdpd_measure_peaks", "tdpd_launch_count",
     "tdpd_set_tuning", "tdpd_set_neighbor_list", "tdpd_set_membrane_variant", "tdpd_get_neighbor_list_stats", "tdpd_set_graph", "tdpd_last_error", "tdpd_destroy",
+    "tdpd_noalloc_init", "tdpd_sort_cells_noalloc", "tdpd_noalloc_last_error",
 )
 
 
@@ -64,6 +65,28 @@ def measure_peaks(device: int = 0) -> dict:
     if rc != OK:
         raise TdpdError(rc, "tdpd_measure_peaks failed")
     return {k: getattr(pk, k) for k, _ in Peaks._fields_ if k != "reserved"}
+
+
+NOALLOC_MAX_N = 262144  # TDPD_NOALLOC_MAX_N
+
+
+def noalloc_init() -> None:
+    """tdpd_noalloc_init: looks up the fixed sort scratch on the current CUDA device (call before a stream capture)."""
+    L = load_library()
+    rc = L.tdpd_noalloc_init()
+    if rc != OK:
+        raise TdpdError(rc, L.tdpd_noalloc_last_error().decode())
+
+
+def sort_cells_noalloc(d_keys: int, d_vals: int, n: int, key_bits: int, d_keys_out: int, d_vals_out: int,
+                       stream: int = 0) -> None:
+    """tdpd_sort_cells_noalloc: stable radix sort of n (key, value) pairs given as DEVICE addresses (ints; d_vals = 0
+    for the values 0 .. n-1), scratch in a fixed device array of the library, no allocation; enqueues on `stream`."""
+    L = load_library()
+    rc = L.tdpd_sort_cells_noalloc(C.c_void_p(d_keys), C.c_void_p(d_vals or None), int(n), int(key_bits),
+                                   C.c_void_p(d_keys_out), C.c_void_p(d_vals_out), C.c_void_p(stream or None))
+    if rc != OK:
+        raise TdpdError(rc, L.tdpd_noalloc_last_error().decode())
 
 
 def make_params(p: dict) -> Params:
@@ -148,6 +171,10 @@ def load_library() -> C.CDLL:
     L.tdpd_last_error.argtypes = [vp]
     L.tdpd_last_error.restype = C.c_char_p
     L.tdpd_destroy.argtypes = [vp]
+    L.tdpd_noalloc_init.argtypes = []
+    L.tdpd_sort_cells_noalloc.argtypes = [vp, vp, i64, i32, vp, vp, vp]
+    L.tdpd_noalloc_last_error.argtypes = []
+    L.tdpd_noalloc_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         getattr(L, name)  # AttributeError if the library does not export a declared symbol
     _lib = L

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtdpd.so")
-SOURCES = ["api.cu", "integrate.cu", "binning.cu", "pair.cu", "pair_s1.cu", "pair_s2.cu", "pair_s4.cu", "pair_s16.cu", "pair_l1.cu", "pair_list.cu", "membrane.cu", "debug.cu", "peaks.cu"]
+SOURCES = ["api.cu", "integrate.cu", "binning.cu", "pair.cu", "pair_s1.cu", "pair_s2.cu", "pair_s4.cu", "pair_s16.cu", "pair_l1.cu", "pair_list.cu", "membrane.cu", "debug.cu", "peaks.cu", "sort_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [f"-D{k}={v}" for k, v in os.environ.items() if k.startswith("TD_PAIR_")] + ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
