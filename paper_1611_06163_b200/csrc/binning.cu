@@ -98,7 +98,11 @@ __global__ void __launch_bounds__(1024) k_sort_scan_tops(uint32_t* __restrict__ 
 }
 
 // stable scatter: tile order = (warp, item, lane); rank = scanned tile base + keys of the same digit in earlier
-// warps of the tile + earlier keys of the same digit in this warp
+// warps of the tile + earlier keys of the same digit in this warp.  The tile is first put in digit order in shared
+// memory (local rank = start of the digit inside the tile + the same two terms), then written out by consecutive
+// threads: keys of one digit leave as one contiguous run (~16 keys = 64 B for a uniform digit) instead of 4-byte stores
+// from 32 lanes to 32 different sectors (round 2, 6.9 M keys: the three passes of a binning 0.287 -> 0.273 ms; what
+// remains is the 16 MATCH.ANY per thread: replacing the shared atomics of the counting by more of them made it slower).
 __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __restrict__ kin,
                                                           const uint32_t* __restrict__ vin,
                                                           uint32_t* __restrict__ kout, uint32_t* __restrict__ vout,
@@ -107,10 +111,14 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
                                                           const uint32_t* __restrict__ gate) {
   TD_GATE(gate);
   __shared__ uint32_t wbase[SORT_NT / 32][NBIN];
+  __shared__ uint32_t gdelta[NBIN];  // global position of a key = its position in the digit-ordered tile + gdelta[digit]
+  __shared__ uint32_t wsum[SORT_NT / 32];
+  __shared__ uint32_t skey[TILE], sval[TILE];
   int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int k = threadIdx.x; k < (SORT_NT / 32) * NBIN; k += SORT_NT) (&wbase[0][0])[k] = 0;
   __syncthreads();
-  int64_t base = (int64_t)blockIdx.x * TILE + (int64_t)w * WCHUNK;
+  const int64_t tile0 = (int64_t)blockIdx.x * TILE;
+  int64_t base = tile0 + (int64_t)w * WCHUNK;
   uint32_t key[SORT_ITEMS];
 #pragma unroll
   for (int it = 0; it < SORT_ITEMS; ++it) {
@@ -119,15 +127,29 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
     if (i < n) atomicAdd(&wbase[w][(key[it] >> shift) & (NBIN - 1)], 1u);
   }
   __syncthreads();
-  {  // per bin: counts -> exclusive prefix over warps + global base
-    int b = threadIdx.x;
+  {  // per bin (thread b owns bin b): tile count -> exclusive scan over the bins = local start of the digit
+    const int b = threadIdx.x;
+    uint32_t c[SORT_NT / 32], tot = 0;
+#pragma unroll
+    for (int ww = 0; ww < SORT_NT / 32; ++ww) { c[ww] = wbase[ww][b]; tot += c[ww]; }
+    uint32_t x = tot;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      uint32_t y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) wsum[w] = x;
+    __syncthreads();
+    uint32_t before = 0;
+#pragma unroll
+    for (int ww = 0; ww < SORT_NT / 32; ++ww) before += ww < w ? wsum[ww] : 0u;
+    uint32_t run = before + x - tot;  // keys of smaller digits in this tile
     const int64_t hi = (int64_t)b * nblk + blockIdx.x;
-    uint32_t run = hist[hi] + tops[hi / SCAN_CHUNK];
+    gdelta[b] = hist[hi] + tops[hi / SCAN_CHUNK] - run;
 #pragma unroll
     for (int ww = 0; ww < SORT_NT / 32; ++ww) {
-      uint32_t c = wbase[ww][b];
       wbase[ww][b] = run;
-      run += c;
+      run += c[ww];
     }
   }
   __syncthreads();
@@ -144,9 +166,18 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __rest
     if (valid && rank == 0) wbase[w][d] += __popc(peers);
     __syncwarp();
     if (valid) {
-      kout[dest] = key[it];
-      vout[dest] = vin[i];
+      skey[dest] = key[it];
+      sval[dest] = vin[i];
     }
+  }
+  __syncthreads();
+  const int nvalid = (int)(n - tile0 < (int64_t)TILE ? n - tile0 : (int64_t)TILE);
+#pragma unroll 4
+  for (int k = threadIdx.x; k < nvalid; k += SORT_NT) {
+    const uint32_t kk = skey[k];
+    const uint32_t pos = (uint32_t)k + gdelta[(kk >> shift) & (NBIN - 1)];
+    kout[pos] = kk;
+    vout[pos] = sval[k];
   }
 }
 
