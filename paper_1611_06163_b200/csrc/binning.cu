@@ -10,6 +10,9 @@ constexpr int SORT_NT = 256;     // 8 warps
 constexpr int SORT_ITEMS = 16;   // keys per thread
 constexpr int TILE = SORT_NT * SORT_ITEMS;
 constexpr int WCHUNK = 32 * SORT_ITEMS;  // contiguous keys owned by one warp
+#ifndef SORT_SCATTER_MINB
+#define SORT_SCATTER_MINB 4  // 64 registers: four CTAs per SM instead of three (round 2, 6.9 M keys, three passes: 0.273 -> 0.239 ms)
+#endif
 
 // per-tile digit histogram -> hist[bin * nblk + blk]  (integer counts: atomics cannot change the result)
 // `gate` (may be NULL): the device control block of the neighbour-list mode; the kernels of the binning return at once
@@ -103,7 +106,7 @@ __global__ void __launch_bounds__(1024) k_sort_scan_tops(uint32_t* __restrict__ 
 // threads: keys of one digit leave as one contiguous run (~16 keys = 64 B for a uniform digit) instead of 4-byte stores
 // from 32 lanes to 32 different sectors (round 2, 6.9 M keys: the three passes of a binning 0.287 -> 0.273 ms; what
 // remains is the 16 MATCH.ANY per thread: replacing the shared atomics of the counting by more of them made it slower).
-__global__ void __launch_bounds__(SORT_NT) k_sort_scatter(const uint32_t* __restrict__ kin,
+__global__ void __launch_bounds__(SORT_NT, SORT_SCATTER_MINB) k_sort_scatter(const uint32_t* __restrict__ kin,
                                                           const uint32_t* __restrict__ vin,
                                                           uint32_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                           int64_t n, int shift, const uint32_t* __restrict__ hist,
