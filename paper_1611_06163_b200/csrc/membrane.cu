@@ -37,7 +37,13 @@ __device__ __forceinline__ float wlc_force(float kBT_over_p, float x) {
   return kBT_over_p * (0.25f / (om * om) - 0.25f + x);
 }
 
-__global__ void __launch_bounds__(256) k_membrane(const __grid_constant__ DevParams P, const MembraneArgs A) {
+// 64 registers (four CTAs per SM) instead of the 128 ptxas takes when left alone (two CTAs, 19 % occupancy): the kernel
+// is bound by fixed-latency and load waits at IPC 1.8, not by registers; config 5: 0.258 -> 0.208 ms alone, the step
+// 6.478 -> 6.433 ms with the kernel beside the pair kernel (3 and 5 CTAs per SM: 6.447 / 6.439)
+#ifndef TD_MEM_MINB
+#define TD_MEM_MINB 4
+#endif
+__global__ void __launch_bounds__(256, TD_MEM_MINB) k_membrane(const __grid_constant__ DevParams P, const MembraneArgs A) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[2][8];
   __shared__ double tot[2];
