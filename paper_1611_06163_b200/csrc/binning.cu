@@ -26,12 +26,32 @@ __global__ void __launch_bounds__(SORT_NT) k_sort_hist(const uint32_t* __restric
   __shared__ uint32_t cnt[NBIN];
   cnt[threadIdx.x] = 0;
   __syncthreads();
-  int64_t base = (int64_t)blockIdx.x * TILE;
-#pragma unroll 4
-  for (int it = 0; it < SORT_ITEMS; ++it) {
-    int64_t i = base + it * SORT_NT + threadIdx.x;
-    if (i < n) atomicAdd(&cnt[(keys[i] >> shift) & (NBIN - 1)], 1u);
+  // every thread takes SORT_ITEMS CONSECUTIVE keys and adds once per run of equal digits: the keys arrive almost
+  // sorted (particles move little in a step), so a thread's 16 keys hold one or two digits in the low passes and the
+  // 32 lanes of a warp no longer queue on one shared-memory word (config 5, three passes: sort 0.218 -> 0.196 ms; config 2: 0.056 -> 0.048 ms)
+  const int64_t i0 = (int64_t)blockIdx.x * TILE + (int64_t)threadIdx.x * SORT_ITEMS;
+  uint32_t k[SORT_ITEMS];
+  if (i0 + SORT_ITEMS <= n && (reinterpret_cast<uintptr_t>(keys) & 15u) == 0) {  // (a caller's array may be 4-byte aligned)
+#pragma unroll
+    for (int q = 0; q < SORT_ITEMS / 4; ++q) {
+      const uint4 v = __ldg(reinterpret_cast<const uint4*>(keys + i0) + q);
+      k[4 * q] = v.x; k[4 * q + 1] = v.y; k[4 * q + 2] = v.z; k[4 * q + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int q = 0; q < SORT_ITEMS; ++q) k[q] = i0 + q < n ? keys[i0 + q] : 0u;
   }
+  const int nv = (int)(n - i0 < (int64_t)SORT_ITEMS ? (n - i0 > 0 ? n - i0 : 0) : (int64_t)SORT_ITEMS);
+  uint32_t dprev = 0, run = 0;
+#pragma unroll
+  for (int q = 0; q < SORT_ITEMS; ++q) {
+    const uint32_t d = (k[q] >> shift) & (NBIN - 1);
+    if (q < nv) {
+      if (run && d != dprev) { atomicAdd(&cnt[dprev], run); run = 0; }
+      dprev = d; ++run;
+    }
+  }
+  if (run) atomicAdd(&cnt[dprev], run);
   __syncthreads();
   hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
 }

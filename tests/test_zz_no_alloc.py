@@ -98,6 +98,15 @@ def test_noalloc_sort_at_the_maximum_size_and_its_limits(T):
         T.sort_cells_noalloc(dk.data_ptr(), 0, m, 32, ok.data_ptr(), ov.data_ptr(), st)
         order = np.argsort(keys[:m], kind="stable")
         assert np.array_equal(host(ov)[:m], order.astype(np.uint32))
+    # arrays that are only 4-byte aligned (views that start one element in), 2 and 3 passes: the sort lands in them
+    for bits in (16, 24):
+        m = 20000
+        kin = keys[1:m + 1] & np.uint32((1 << bits) - 1)
+        dk.view(torch.int32)[1:m + 1].copy_(torch.from_numpy(kin.view(np.int32)))
+        T.sort_cells_noalloc(dk.data_ptr() + 4, 0, m, bits, ok.data_ptr() + 4, ov.data_ptr() + 4, st)
+        order = np.argsort(kin, kind="stable")
+        assert np.array_equal(host(ov)[1:m + 1], order.astype(np.uint32))
+        assert np.array_equal(host(ok)[1:m + 1], kin[order])
     # beyond the maximum: a clear error, nothing enqueued, the outputs keep their contents
     before = host(ov).copy()
     with pytest.raises(T.TdpdError) as e:
