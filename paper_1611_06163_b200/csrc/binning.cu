@@ -143,11 +143,35 @@ __global__ void __launch_bounds__(SORT_NT, SORT_SCATTER_MINB) k_sort_scatter(con
   const int64_t tile0 = (int64_t)blockIdx.x * TILE;
   int64_t base = tile0 + (int64_t)w * WCHUNK;
   uint32_t key[SORT_ITEMS];
+  {  // counts of this warp's 512 keys: every lane takes 16 consecutive ones and adds once per run of equal digits (as
+     // in k_sort_hist); the keys are read again below in the (item, lane) order the ranks need, from L1
+    const int64_t j0 = base + (int64_t)lane * SORT_ITEMS;
+    if (j0 + SORT_ITEMS <= n && (reinterpret_cast<uintptr_t>(kin) & 15u) == 0) {
+#pragma unroll
+      for (int q = 0; q < SORT_ITEMS / 4; ++q) {
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(kin + j0) + q);
+        key[4 * q] = v.x; key[4 * q + 1] = v.y; key[4 * q + 2] = v.z; key[4 * q + 3] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < SORT_ITEMS; ++q) key[q] = j0 + q < n ? kin[j0 + q] : 0u;
+    }
+    const int nv = (int)(n - j0 < (int64_t)SORT_ITEMS ? (n - j0 > 0 ? n - j0 : 0) : (int64_t)SORT_ITEMS);
+    uint32_t dprev = 0, run = 0;
+#pragma unroll
+    for (int q = 0; q < SORT_ITEMS; ++q) {
+      const uint32_t d = (key[q] >> shift) & (NBIN - 1);
+      if (q < nv) {
+        if (run && d != dprev) { atomicAdd(&wbase[w][dprev], run); run = 0; }
+        dprev = d; ++run;
+      }
+    }
+    if (run) atomicAdd(&wbase[w][dprev], run);
+  }
 #pragma unroll
   for (int it = 0; it < SORT_ITEMS; ++it) {
     int64_t i = base + it * 32 + lane;
     key[it] = i < n ? kin[i] : 0xFFFFFFFFu;
-    if (i < n) atomicAdd(&wbase[w][(key[it] >> shift) & (NBIN - 1)], 1u);
   }
   __syncthreads();
   {  // per bin (thread b owns bin b): tile count -> exclusive scan over the bins = local start of the digit
