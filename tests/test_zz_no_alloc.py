@@ -77,6 +77,20 @@ def test_noalloc_sort_matches_the_simulation_sort_twice_in_a_row(T):
     T.sort_cells_noalloc(dk.data_ptr(), 0, n1, bits1, ok.data_ptr(), ov.data_ptr(), st)
     assert np.array_equal(host(ov), sid1) and np.array_equal(host(ok), got_k1)
 
+    # ---- and under stream capture, where an allocation (or any synchronising call) would invalidate the capture:
+    # the call is recorded into a CUDA graph, the outputs are cleared, the graph is replayed twice
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        T.sort_cells_noalloc(dk.data_ptr(), 0, n1, bits1, ok.data_ptr(), ov.data_ptr(), side.cuda_stream)
+    for _ in range(2):
+        ok.zero_(); ov.zero_()
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(host(ov), sid1) and np.array_equal(host(ok), got_k1)
+
 
 def test_noalloc_sort_at_the_maximum_size_and_its_limits(T):
     import torch
