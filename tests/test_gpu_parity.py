@@ -915,3 +915,29 @@ def test_source_term_matches_oracle(T, orc):
     # the totals moved by what the source put in and the decay took out (no longer conserved)
     c0 = w.all_particles()[3].astype(np.float64).sum(axis=0)
     assert np.all(np.abs(g["conc"].astype(np.float64).sum(axis=0) - c0) > 1.0)
+
+
+@pytest.mark.parametrize("c,total", [(3, 20000), (4, 5000), (5, 2000)])
+def test_long_runs_stay_stable(T, c, total):
+    """Beyond BASELINE.json's run lengths (TDPD_SLOW=1; last run: profiles/r2_soak.md): four chunks of total / 4 steps;
+    after each the state must read back clean (tdpd_get_state reports NaN / Inf and overstretched bonds), the total
+    concentration of every species must not drift, every membrane must hold its area and volume."""
+    import os
+    import time
+    if not os.environ.get("TDPD_SLOW"):
+        pytest.skip("long runs: TDPD_SLOW=1 (last run: profiles/r2_soak.md)")
+    w = W.config(c)
+    sim = T.Simulation.from_workload(w)
+    c0 = sim.get_state(forces=False)["conc"].astype(np.float64).sum(0)
+    t0 = time.perf_counter()
+    rows = []
+    for k in range(4):
+        sim.step(total // 4)
+        s = sim.get_state(forces=False)                      # raises on NaN / Inf / overstretched bond
+        drift = np.abs(s["conc"].astype(np.float64).sum(0) / c0 - 1.0).max()
+        st = sim.rbc_stats()
+        da, dv = np.abs(st["area"] / st["A0"] - 1).max(), np.abs(st["volume"] / st["V0"] - 1).max()
+        rows.append((s["step"], drift, da, dv))
+        assert drift < 1e-5 and da < 1e-2 and dv < 1e-2, rows
+    print(f"[soak] config{c}: " + "; ".join(f"step {a}: conc drift {b:.1e}, dA {d:.1e}, dV {e:.1e}" for a, b, d, e in rows)
+          + f"; wall {time.perf_counter() - t0:.1f} s")
