@@ -59,3 +59,22 @@ def test_product_never_imports_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "tdpd_oracle" not in txt, f
+
+
+def test_noalloc_sort_argument_checks_need_no_gpu(T):
+    """tdpd_sort_cells_noalloc refuses bad sizes before it touches CUDA: checked here without a device; the binding's
+    limit is the header's."""
+    hdr = open(os.path.join(ROOT, "include", "tdpd.h")).read()
+    assert int(re.search(r"#define TDPD_NOALLOC_MAX_N (\d+)", hdr).group(1)) == T.NOALLOC_MAX_N
+    scratch = int(re.search(r"#define TDPD_NOALLOC_SCRATCH_BYTES (\d+)", hdr).group(1))
+    assert scratch == 2 * 4 * T.NOALLOC_MAX_N + 128 * 1024
+    with pytest.raises(T.TdpdError) as e:
+        T.sort_cells_noalloc(256, 0, T.NOALLOC_MAX_N + 1, 16, 256, 256)
+    assert e.value.code == -1 and "TDPD_NOALLOC_MAX_N" in str(e.value)
+    for n, bits in ((-1, 16), (16, 0), (16, 33)):
+        with pytest.raises(T.TdpdError) as e:
+            T.sort_cells_noalloc(256, 0, n, bits, 256, 256)
+        assert e.value.code == -1
+    T.sort_cells_noalloc(0, 0, 0, 16, 0, 0)      # n = 0 is a no-op, also without a device
+    with pytest.raises(T.TdpdError):
+        T.sort_cells_noalloc(0, 0, 16, 16, 256, 256)   # NULL keys
